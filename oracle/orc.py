@@ -1,0 +1,122 @@
+"""ctypes wrapper of the oracle library (TEST INFRASTRUCTURE; see z4c_oracle.hpp).
+
+May be imported only by tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference leg. It takes numpy arrays and plain patch
+descriptors (any object with nx ny nz pitch_x field_stride patch_offset dx dt).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import sys
+
+import numpy as np
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+import build as _build  # noqa: E402  (oracle/build.py)
+
+NF = 25
+
+
+class OrcPatch(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("ng", C.c_int32),
+                ("pitch_x", C.c_int64), ("field_stride", C.c_int64), ("patch_offset", C.c_int64),
+                ("dx", C.c_double), ("dt", C.c_double)]
+
+
+class OrcParams(C.Structure):
+    _fields_ = [("kappa1", C.c_double), ("kappa2", C.c_double), ("eta", C.c_double),
+                ("shift_coef", C.c_double), ("ko_sigma", C.c_double),
+                ("lapse_uses_khat", C.c_int32)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.orc_num_threads.restype = C.c_int
+    return _lib
+
+
+def _patches(ps):
+    arr = (OrcPatch * len(ps))()
+    for a, p in zip(arr, ps):
+        a.nx, a.ny, a.nz, a.ng = p.nx, p.ny, p.nz, 3
+        a.pitch_x, a.field_stride, a.patch_offset = p.pitch_x, p.field_stride, p.patch_offset
+        a.dx, a.dt = p.dx, p.dt
+    return arr
+
+
+def _params(d):
+    return OrcParams(d["kappa1"], d["kappa2"], d["eta"], d["shift_coef"], d["ko_sigma"],
+                     int(d.get("lapse_uses_khat", 1)))
+
+
+def _p(a):
+    assert a.dtype == np.float64 and a.flags.c_contiguous
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def num_threads() -> int:
+    return lib().orc_num_threads()
+
+
+def set_threads(n: int):
+    lib().orc_set_threads(int(n))
+
+
+def fill_ghosts(ps, u):
+    lib().orc_fill_ghosts(_patches(ps), len(ps), _p(u))
+
+
+def z4c_rhs(ps, prm, u, quad=False):
+    """RHS (incl. KO) on the active cells of a ghost-filled state; zeros elsewhere."""
+    rhs = np.zeros_like(u)
+    pr = _params(prm)
+    if quad:
+        lib().orc_z4c_rhs_q(_patches(ps), len(ps), C.byref(pr), _p(u), _p(rhs), C.c_int64(u.size))
+    else:
+        lib().orc_z4c_rhs(_patches(ps), len(ps), C.byref(pr), _p(u), _p(rhs))
+    return rhs
+
+
+def rk4_substep(ps, prm, stage, u_n, u_in, u_out, acc):
+    kbuf = np.zeros_like(u_in)
+    pr = _params(prm)
+    lib().orc_rk4_substep(_patches(ps), len(ps), C.byref(pr), int(stage), _p(u_n), _p(u_in),
+                          _p(u_out), _p(acc), _p(kbuf))
+
+
+def rk4_step(ps, prm, u, quad=False):
+    """Advance u in place by one RK4 step (ghosts filled on return).
+    Returns S, the increment per unit dt, on active cells (zeros elsewhere)."""
+    pr = _params(prm)
+    n = u.size
+    if quad:
+        S = np.zeros_like(u)
+        lib().orc_rk4_step_q(_patches(ps), len(ps), C.byref(pr), _p(u), _p(S), C.c_int64(n))
+        return S
+    work = np.zeros(4 * n)
+    lib().orc_rk4_step(_patches(ps), len(ps), C.byref(pr), _p(u), _p(work), C.c_int64(n))
+    return work[2 * n:3 * n].copy()
+
+
+def rhs_point(prm, u, d1, d2, adv, ko):
+    """Point-wise algebra with caller-supplied derivatives. u[25], d1[25,3], d2[25,6]."""
+    u, d1, d2, adv, ko = (np.ascontiguousarray(a, dtype=np.float64) for a in (u, d1, d2, adv, ko))
+    assert u.shape == (NF,) and d1.shape == (NF, 3) and d2.shape == (NF, 6)
+    out = np.zeros(NF)
+    pr = _params(prm)
+    lib().orc_rhs_point(C.byref(pr), _p(u), _p(d1), _p(d2), _p(adv), _p(ko), _p(out))
+    return out
+
+
+def derivs_field(p, u, f, i, j, k, sigma):
+    """(d1[3], d2[6], adv, ko) of field f at active cell (i,j,k) of patch p."""
+    out = np.zeros(11)
+    lib().orc_derivs_field(C.byref(_patches([p])[0]), _p(u), int(f), int(i), int(j), int(k),
+                           C.c_double(sigma), _p(out))
+    return out[0:3], out[3:9], out[9], out[10]

@@ -1,0 +1,104 @@
+// z4c_oracle_capi.cpp -- TEST INFRASTRUCTURE (the oracle's own C interface).
+//
+// extern "C" entry points over the templated oracle, as double (the oracle) and
+// as __float128 (referee: same source, 113-bit significand, inputs/outputs
+// converted from/to double at the interface). Built by oracle/build.py with
+//   g++ -O2 -std=c++17 -fopenmp -ffp-contract=off -fno-fast-math -shared -fPIC
+// (the paper's flags: PAPER.md:206).
+// This library is NOT the product's C ABI (that is include/sacra.h) and shares
+// no code with it.
+#include <cstring>
+#include <vector>
+#include <omp.h>
+#include "z4c_grid.hpp"
+
+using namespace z4c_oracle;
+
+extern "C" {
+struct orc_patch { int32_t nx, ny, nz, ng; int64_t pitch_x, field_stride, patch_offset; double dx, dt; };
+struct orc_params { double kappa1, kappa2, eta, shift_coef, ko_sigma; int32_t lapse_uses_khat; };
+}
+
+static Patch to_patch(const orc_patch& q) {
+  Patch p; p.nx = q.nx; p.ny = q.ny; p.nz = q.nz; p.pitch = q.pitch_x; p.fstride = q.field_stride;
+  p.offset = q.patch_offset; p.dx = q.dx; p.dt = q.dt; return p;
+}
+template <class T> static Params<T> to_params(const orc_params& q) {
+  Params<T> P; P.kappa1 = T(q.kappa1); P.kappa2 = T(q.kappa2); P.eta = T(q.eta);
+  P.shift_coef = T(q.shift_coef); P.ko_sigma = T(q.ko_sigma); P.lapse_uses_khat = q.lapse_uses_khat;
+  return P;
+}
+
+extern "C" {
+
+int orc_num_threads(void) { return omp_get_max_threads(); }
+void orc_set_threads(int n) { omp_set_num_threads(n); }
+
+// ---- double ---------------------------------------------------------------
+void orc_fill_ghosts(const orc_patch* ps, int np, double* u) {
+  for (int q = 0; q < np; ++q) fill_ghosts<double>(to_patch(ps[q]), u);
+}
+void orc_z4c_rhs(const orc_patch* ps, int np, const orc_params* prm, const double* u, double* rhs) {
+  auto P = to_params<double>(*prm);
+  for (int q = 0; q < np; ++q) rhs_patch<double>(to_patch(ps[q]), P, u, rhs);
+}
+// stage in 1..4; kbuf: scratch state of the same size
+void orc_rk4_substep(const orc_patch* ps, int np, const orc_params* prm, int stage, const double* u_n,
+                     const double* u_in, double* u_out, double* acc, double* kbuf) {
+  auto P = to_params<double>(*prm);
+  for (int q = 0; q < np; ++q) rk4_substep<double>(to_patch(ps[q]), P, stage, u_n, u_in, u_out, acc, kbuf);
+}
+// work: 4 states back to back, each nstate doubles: stage A, stage B, acc (returns S), k scratch
+void orc_rk4_step(const orc_patch* ps, int np, const orc_params* prm, double* u, double* work, int64_t nstate) {
+  auto P = to_params<double>(*prm);
+  std::vector<Patch> v; for (int q = 0; q < np; ++q) v.push_back(to_patch(ps[q]));
+  rk4_step<double>(v.data(), np, P, u, work, work + nstate, work + 2 * nstate, work + 3 * nstate);
+}
+
+// single-point algebra with caller-supplied derivatives (for analytic-derivative pins)
+// d1: [25][3], d2: [25][6] (xx xy xz yy yz zz), adv: [25], ko: [25]
+void orc_rhs_point(const orc_params* prm, const double* u, const double* d1, const double* d2,
+                   const double* adv, const double* ko, double* out) {
+  auto P = to_params<double>(*prm);
+  Derivs<double> D;
+  std::memcpy(D.d1, d1, sizeof(D.d1)); std::memcpy(D.d2, d2, sizeof(D.d2));
+  std::memcpy(D.adv, adv, sizeof(D.adv)); std::memcpy(D.ko, ko, sizeof(D.ko));
+  z4c_rhs_point<double>(u, D, P, out);
+}
+
+// per-point derivative bundle of one field at one active cell (stencil pins)
+// out: d1[3], d2[6], adv, ko  (11 doubles)
+void orc_derivs_field(const orc_patch* p_, const double* u, int field, int i, int j, int k,
+                      double sigma, double* out) {
+  Patch p = to_patch(*p_);
+  const double* f[NF];
+  for (int n = 0; n < NF; ++n) f[n] = u + p.offset + (long)n * p.fstride;
+  Derivs<double> D;
+  derivs_at<double>(f, cell(p, i + NG, j + NG, k + NG), sy_of(p), sz_of(p), p.dx, sigma, D);
+  for (int a = 0; a < 3; ++a) out[a] = D.d1[field][a];
+  for (int a = 0; a < 6; ++a) out[3 + a] = D.d2[field][a];
+  out[9] = D.adv[field]; out[10] = D.ko[field];
+}
+
+// ---- __float128 referee ------------------------------------------------------
+typedef __float128 Q;
+void orc_z4c_rhs_q(const orc_patch* ps, int np, const orc_params* prm, const double* u, double* rhs,
+                   int64_t nstate) {
+  auto P = to_params<Q>(*prm);
+  std::vector<Q> uq(nstate), rq(nstate, Q(0));
+  for (int64_t i = 0; i < nstate; ++i) uq[i] = Q(u[i]);
+  for (int q = 0; q < np; ++q) rhs_patch<Q>(to_patch(ps[q]), P, uq.data(), rq.data());
+  for (int64_t i = 0; i < nstate; ++i) rhs[i] = (double)rq[i];
+}
+void orc_rk4_step_q(const orc_patch* ps, int np, const orc_params* prm, double* u, double* S,
+                    int64_t nstate) {
+  auto P = to_params<Q>(*prm);
+  std::vector<Patch> v; for (int q = 0; q < np; ++q) v.push_back(to_patch(ps[q]));
+  std::vector<Q> uq(nstate), w(4 * nstate, Q(0));
+  for (int64_t i = 0; i < nstate; ++i) uq[i] = Q(u[i]);
+  rk4_step<Q>(v.data(), np, P, uq.data(), w.data(), w.data() + nstate, w.data() + 2 * nstate,
+              w.data() + 3 * nstate);
+  for (int64_t i = 0; i < nstate; ++i) { u[i] = (double)uq[i]; S[i] = (double)w[2 * nstate + i]; }
+}
+
+}  // extern "C"
