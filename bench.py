@@ -1,0 +1,322 @@
+#!/usr/bin/env python
+"""bench.py -- Z4c RHS + KO + RK4 throughput of libsacra on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+One "step" = one full RK4 step (5 halo fills + 4 fused RHS/KO/RK substages) of the whole workload through the
+C ABI call sacra_rk4_step. Default workload: BASELINE.json configs[4], one 256^3 periodic patch, 25 FP64 fields,
+Brill-Lindquist data + 1e-12 seeded noise (the configuration the north_star target is stated on; it fits one
+GPU). N > 1 (torchrun): "replicas only" -- every rank advances its own independent 256^3 patch, no data-path
+collective (Multi-GPU); value = points of all ranks / max-over-ranks time.
+
+Prints ONE JSON line (rank 0). Keys: see DESIGN.md "Measurement".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "Z4c RHS+RK4 Mpoint-updates/s FP64"
+UNIT = "Mpoint-updates/s"
+NF = 25
+# Algorithmic work per point: 16 field passes x 8 B x 25 fields per RK4 step,
+# i.e. 800 B per substage launch on average; FP64 operations per RHS evaluation + RK update (FMA = 2).
+ALG_BYTES_PER_POINT_STEP = 16 * 8 * NF
+ALG_FLOP_PER_POINT_STAGE = 4560.0
+FP64_LANES_PER_SM, N_SM = 64, 148
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
+
+    def stop(self, t0=None, t1=None):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for (t, r) in self.rows if (t0 is None or t >= t0 - 0.05) and (t1 is None or t <= t1 + 0.05)]
+        rows = rows or [r for (_, r) in self.rows]
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_workload(idx: int, n: int | None):
+    from paper_2607_08743_b200 import workloads as wl
+    kw = {}
+    if n:
+        kw["n"] = n
+    return wl.make(idx, **kw)
+
+
+def oracle_sample(w, n_sample: int):
+    """Bounded sample of the workload for the CPU legs: the central n_sample^3 block of patch 0 (same data,
+    same spacing and parameters), advanced as its own periodic patch. Same work per point as the full run."""
+    import numpy as np
+    from paper_2607_08743_b200 import workloads as wl
+    p = w.patches[0]
+    m = min(n_sample, p.nx, p.ny, p.nz)
+    ps, total = wl.make_layout([(m, m, m)], [p.dx], [p.dt], [(0.0, 0.0, 0.0)])
+    s = wl.Workload("sample", ps, dict(w.params), np.zeros(total))
+    o = [(d - m) // 2 for d in (p.nz, p.ny, p.nx)]
+    for f in range(NF):
+        s.active_view(s.state, 0, f)[...] = w.active_view(w.state, 0, f)[o[0]:o[0] + m, o[1]:o[1] + m, o[2]:o[2] + m]
+    return s
+
+
+def time_oracle(sample, steps, warmup):
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import orc
+    u = sample.state.copy()
+    for _ in range(warmup):
+        orc.rk4_step(sample.patches, sample.params, u)
+    ts = []
+    for _ in range(steps):
+        t = time.perf_counter()
+        orc.rk4_step(sample.patches, sample.params, u)
+        ts.append(time.perf_counter() - t)
+    return ts, orc.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = make_workload(args.config, args.n)
+    m = args.oracle_n or 64
+    s = oracle_sample(w, m)
+    ts, cores = time_oracle(s, args.steps, args.warmup)
+    tot = sum(ts)
+    val = s.npoints * len(ts) / tot / 1e6
+    sample = "central %d^3 block of %s as a periodic patch, %d RK4 steps" % (s.patches[0].nx, w.name, len(ts))
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(ts),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2607_08743_b200 import sacra
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libsacra has no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    w = make_workload(args.config, args.n)
+    ps, prm = sacra.make_patches(w.patches), sacra.make_params(w.params)
+    npts = w.npoints
+    n = w.state.size
+    host_in = torch.from_numpy(w.state).pin_memory()
+    host_out = torch.empty_like(host_in).pin_memory()
+    u = torch.empty(n, dtype=torch.float64, device="cuda")
+    work = torch.zeros(3 * n, dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+    K, W = args.steps, args.warmup
+
+    def ev():
+        return torch.cuda.Event(enable_timing=True)
+
+    # ---- device-resident throughput: K consecutive steps, state stays in HBM -----------------------------
+    u.copy_(host_in)
+    for _ in range(W):
+        sacra.rk4_step(ps, prm, u, work, n)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    barrier()
+    t0 = time.time()
+    evs = [ev() for _ in range(K + 1)]
+    evs[0].record(stream)
+    for s in range(K):
+        sacra.rk4_step(ps, prm, u, work, n)
+        evs[s + 1].record(stream)
+    barrier()
+    t1 = time.time()
+    step_ms = [evs[s].elapsed_time(evs[s + 1]) for s in range(K)]
+    total_ms = max_over_ranks(evs[0].elapsed_time(evs[K]))
+    clocks = sampler.stop(t0, t1) if rank == 0 else None
+    if not bool(torch.isfinite(u).all()):
+        raise SystemExit("bench.py: non-finite state after the timed steps")
+
+    # ---- kernel split for the roofline: same nine calls, CUDA events around each -----------------------
+    a, b, acc = work[:n], work[n:2 * n], work[2 * n:]
+    seq = [(u, a), (a, b), (b, a), (a, u)]
+    fill_ms, sub_ms = [], []
+    for it in range(W + K):
+        marks = []
+        for stage, (src, dst) in enumerate(seq, start=1):
+            e = [ev(), ev(), ev()]
+            e[0].record(stream)
+            sacra.fill_ghosts(ps, src)
+            e[1].record(stream)
+            sacra.rk4_substep(ps, prm, stage, u, src, dst, acc)
+            e[2].record(stream)
+            marks.append(e)
+        e = [ev(), ev()]
+        e[0].record(stream); sacra.fill_ghosts(ps, u); e[1].record(stream)
+        torch.cuda.synchronize()
+        if it >= W:
+            fill_ms += [m[0].elapsed_time(m[1]) for m in marks] + [e[0].elapsed_time(e[1])]
+            sub_ms += [m[1].elapsed_time(m[2]) for m in marks]
+    sub_avg = sum(sub_ms) / len(sub_ms)
+    fill_avg = sum(fill_ms) / len(fill_ms)
+
+    # ---- end to end with HOST buffers: H2D of the state, one step, D2H of the new state, every step ----
+    barrier()
+    e0, e1 = ev(), ev()
+    for it in range(min(W, 2) + K):
+        if it == min(W, 2):
+            barrier()
+            e0.record(stream)
+        u.copy_(host_in, non_blocking=True)
+        sacra.rk4_step(ps, prm, u, work, n)
+        host_out.copy_(u, non_blocking=True)
+    e1.record(stream)
+    barrier()
+    e2e_ms = max_over_ranks(e0.elapsed_time(e1))
+
+    if world > 1:
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+
+    hbm_gbs, sm_max_mhz, peak_src = _peaks()
+    value = world * npts * K / (total_ms * 1e-3) / 1e6
+    e2e_val = world * npts * K / (e2e_ms * 1e-3) / 1e6
+    # roofline of the dominant kernel (the fused substage kernel), per launch, averaged over the 4 stages
+    alg_bytes = ALG_BYTES_PER_POINT_STEP / 4.0 * npts
+    alg_flop = ALG_FLOP_PER_POINT_STAGE * npts
+    fp64_peak_tf = N_SM * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    t_hbm = alg_bytes / (hbm_gbs * 1e9)
+    t_alu = alg_flop / (fp64_peak_tf * 1e12)
+    t_k = sub_avg * 1e-3
+    if t_alu >= t_hbm:
+        roof = {"bound": "alu", "achieved": alg_flop / t_k / 1e12, "peak": fp64_peak_tf, "unit": "TFLOP/s"}
+    else:
+        roof = {"bound": "hbm", "achieved": alg_bytes / t_k / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof.update({
+        "traffic": args.traffic, "kernel": "k_z4c (fused derivative+algebra+KO+RK substage)",
+        "kernel_ms": sub_avg, "kernel_share_of_step": 4 * sub_avg / (4 * sub_avg + 5 * fill_avg),
+        "fill_ms": fill_avg, "alg_bytes_per_launch": alg_bytes, "alg_flop_per_launch": alg_flop,
+        "hbm_frac": (alg_bytes / t_k / 1e9) / hbm_gbs, "alu_frac": (alg_flop / t_k / 1e12) / fp64_peak_tf,
+        "peak_source": peak_src + "; FP64 peak = 148 SM x 64 lanes x 2 x sm_max_mhz (DESIGN.md)"})
+
+    # ---- CPU oracle beside it (reported baseline, bounded sample) -----------------------------------------
+    cpu = None
+    if not args.no_cpu:
+        s = oracle_sample(w, args.oracle_n or 96)
+        ts, cores = time_oracle(s, 1, 1 if s.npoints <= 64 ** 3 else 0)
+        cpu = {"value": s.npoints / ts[0] / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "central %d^3 block of %s as a periodic patch, 1 RK4 step (%.1f s)"
+                         % (s.patches[0].nx, w.name, ts[0])}
+
+    state_bytes = n * 8
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": total_ms / K, "ms_per_step_min": min(step_ms), "ms_per_step_median": sorted(step_ms)[K // 2],
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "patches": len(w.patches), "points": npts, "fields": NF, "ghosts": 3,
+                   "state_bytes": state_bytes, "l2": "state (%.2f GB) larger than L2; no flush needed" %
+                   (state_bytes / 1e9) if state_bytes > 2.6e8 else "state fits L2: numbers are L2-resident",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes,
+                "ms_per_step": e2e_ms / K},
+        "gpu_launches": 9 * K, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
+    }
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4: 256^3)")
+    ap.add_argument("--n", type=int, default=None, help="override the grid size (testing only)")
+    ap.add_argument("--oracle-n", type=int, default=None, help="edge of the CPU oracle's sample block")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per launch of the dominant kernel from the committed ncu capture")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

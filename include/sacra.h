@@ -1,0 +1,114 @@
+/* sacra.h -- C ABI of libsacra: the B200-native (sm_100a) hot path of SACRA-K's spacetime
+ * evolution (arxiv/paper_2607_08743): periodic halo fill, Z4c/BSSN right-hand side with 4th-order
+ * finite differences, upwind shift advection and 6th-derivative Kreiss-Oliger dissipation, and the
+ * classical RK4 update, on batches of independent uniform FP64 patches.
+ *
+ * Citations: PAPER.md:N is a line of the paper's text; "SURVEY 8(c) item k" is the written-out form of
+ * the system in SURVEY.md (the paper defers the equations to Hilditch et al. 2013).
+ *
+ * Conventions common to every call
+ *   - All state pointers (u, rhs, u_n, u_in, u_out, acc, work) are DEVICE pointers to FP64 data, 16-byte
+ *     aligned, owned by the caller. The library allocates nothing and keeps no pointer after return.
+ *   - `p` (npatch patch descriptors) and `prm` are HOST pointers, read during the call only.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream). Every call only
+ *     enqueues work on that stream; no call synchronises the device or the stream.
+ *   - A "state" is one buffer holding, for every patch, SACRA_NF = 25 fields. Field f of a patch starts at
+ *     base + patch_offset + f*field_stride (in doubles) and is a (nz+2ng) x (ny+2ng) x pitch_x array, x
+ *     fastest; active cell (i,j,k) is stored at ((k+ng)*(ny+2ng) + (j+ng))*pitch_x + (i+ng).
+ *     All states passed to one call share the same layout (the same descriptors address each of them).
+ *   - Return value: SACRA_OK (0) or a negative sacra_status. No exceptions cross the ABI; nothing is
+ *     written to stdout/stderr. NaN/Inf in the data are not detected.
+ *
+ * Field order (SURVEY 8 conventions):
+ *   0 W | 1-6 gt_xx gt_xy gt_xz gt_yy gt_yz gt_zz | 7 K-hat | 8-13 At_xx..At_zz (same order) |
+ *   14-16 Gt^x Gt^y Gt^z | 17 Theta | 18 alpha | 19-21 beta^x..z | 22-24 B^x..z
+ */
+#ifndef SACRA_H_
+#define SACRA_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SACRA_NF 25 /* evolved fields: 1+6+1+6+3+1+1+3+3 */
+#define SACRA_NG 3  /* ghost zones per side: reach of the upwind and KO stencils */
+
+typedef enum {
+  SACRA_OK = 0,
+  SACRA_ERR_NULL = -1,        /* a required pointer is NULL                                        */
+  SACRA_ERR_BADARG = -2,      /* n < 6, dx <= 0, non-finite dx/dt, stage outside 1..4, npatch < 1,
+                                 pitch/stride/offset too small or negative, forbidden aliasing      */
+  SACRA_ERR_UNSUPPORTED = -3, /* ng != 3                                                           */
+  SACRA_ERR_ALIGN = -4,       /* pointer not 16-byte aligned, or pitch_x/field_stride/patch_offset
+                                 breaks the 16-byte row alignment rule below                       */
+  SACRA_ERR_CUDA = -5         /* a CUDA launch failed (cudaGetLastError)                           */
+} sacra_status;
+
+/* One uniform, cell-centred patch (every box of the hierarchy is such a patch). */
+typedef struct {
+  int32_t nx, ny, nz;   /* active cells per axis, each >= 6                                          */
+  int32_t ng;           /* ghost zones per side; must be 3                                           */
+  int64_t pitch_x;      /* doubles per x-row, >= nx + 2*ng, even (rows start 16-byte aligned)        */
+  int64_t field_stride; /* doubles between consecutive fields, >= pitch_x*(ny+2ng)*(nz+2ng), even    */
+  int64_t patch_offset; /* doubles from a state's base pointer to field 0 of this patch, >= 0;
+                           (patch_offset + ng) must be even, so that active cell i=0 of every row is
+                           16-byte aligned                                                           */
+  double dx;            /* grid spacing, dx = dy = dz > 0                                            */
+  double dt;            /* full RK4 step of this patch (Courant factor times dx)        */
+} sacra_patch_t;
+
+/* Parameters of the evolution system. */
+typedef struct {
+  double kappa1, kappa2;   /* Z4c constraint damping                    */
+  double eta;              /* Gamma-driver damping, Eq. 8                             */
+  double shift_coef;       /* coefficient of B^i in Eq. 7: 0.75                       */
+  double ko_sigma;         /* Kreiss-Oliger strength; Q = sigma h^5/64 (D+D-)^3       */
+  int32_t lapse_uses_khat; /* Eq. 6 source: 1 -> -2 alpha K-hat (default reading),
+                              0 -> -2 alpha (K-hat + 2 Theta)                                       */
+  int32_t reserved_;       /* set to 0                                                              */
+} sacra_params_t;
+
+/* Periodic halo fill (stands in for the paper's ghost exchange).
+ * For every field of every patch, each storage cell with an index outside the active range takes the
+ * value of the active cell with per-axis wrapped index; faces, edges and corners. In place on u. Pitch
+ * padding beyond nx+2ng is not touched. */
+int sacra_fill_ghosts(const sacra_patch_t* p, int npatch, double* u, void* cuda_stream);
+
+/* Z4c right-hand side including KO dissipation, F(u) (PAPER.md:49-73,
+ * PAPER.md:99). u: ghosts already filled (read only). rhs: the 25 RHS values are written on active cells;
+ * ghost cells and padding of rhs are not touched. rhs must not alias u. */
+int sacra_z4c_rhs(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, const double* u,
+                  double* rhs, void* cuda_stream);
+
+/* One classical RK4 substage. With k = F(u_in) on active cells:
+ *   stage 1: u_out = u_n + (dt/2) k ; acc  = k          (requires u_in = u_n)
+ *   stage 2: u_out = u_n + (dt/2) k ; acc += 2k
+ *   stage 3: u_out = u_n + dt k     ; acc += 2k
+ *   stage 4: S = (acc + k) * (1/6)  ; u_out = u_n + dt S ; acc = S
+ * u_in: ghosts filled (read through the stencil). u_n: read at active cells only. u_out, acc: active
+ * cells written, ghosts not touched. u_out must not alias u_in; u_out may alias u_n (centre-only access);
+ * acc must alias none of the others. At stage 1 acc is write-only. */
+int sacra_rk4_substep(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, int stage,
+                      const double* u_n, const double* u_in, double* u_out, double* acc,
+                      void* cuda_stream);
+
+/* One full RK4 step: for s = 1..4 { fill_ghosts(stage input); rk4_substep(s) }; fill_ghosts(result).
+ * u: in = state n (ghosts need not be filled), out = state n+1 with ghosts filled.
+ * work: 3 states back to back, each `state_doubles` long (two stage buffers and acc). On return
+ * work + 2*state_doubles holds S, the increment per unit dt, on active cells. Bitwise identical to the
+ * nine-call sequence above. */
+int sacra_rk4_step(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, double* u,
+                   double* work, int64_t state_doubles, void* cuda_stream);
+
+/* Static description of a status code (never NULL). */
+const char* sacra_strerror(int code);
+
+/* Library version, "major.minor" */
+const char* sacra_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SACRA_H_ */

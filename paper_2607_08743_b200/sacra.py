@@ -1,0 +1,144 @@
+"""ctypes binding of libsacra (include/sacra.h): argument marshalling only.
+
+Same names as the C ABI. State arguments are torch CUDA float64 tensors (or raw device pointers as
+ints); every step of the path runs in the CUDA kernels of libsacra. There is no CPU fallback: if the
+library cannot be built or loaded, importing this module raises.
+
+    from paper_2607_08743_b200 import sacra
+    sacra.rk4_step(patches, params, u, work)          # enqueues on torch's current CUDA stream
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+from . import build as _build
+
+NF = 25
+NG = 3
+OK, ERR_NULL, ERR_BADARG, ERR_UNSUPPORTED, ERR_ALIGN, ERR_CUDA = 0, -1, -2, -3, -4, -5
+EXPORTS = ("sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4_step",
+           "sacra_strerror", "sacra_version")
+
+
+class SacraPatch(C.Structure):
+    """sacra_patch_t"""
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("ng", C.c_int32),
+                ("pitch_x", C.c_int64), ("field_stride", C.c_int64), ("patch_offset", C.c_int64),
+                ("dx", C.c_double), ("dt", C.c_double)]
+
+
+class SacraParams(C.Structure):
+    """sacra_params_t"""
+    _fields_ = [("kappa1", C.c_double), ("kappa2", C.c_double), ("eta", C.c_double),
+                ("shift_coef", C.c_double), ("ko_sigma", C.c_double),
+                ("lapse_uses_khat", C.c_int32), ("reserved_", C.c_int32)]
+
+
+class SacraError(RuntimeError):
+    def __init__(self, code: int):
+        self.code = code
+        super().__init__("libsacra: %s (%d)" % (strerror(code), code))
+
+
+def _load():
+    # SACRA_LIB overrides the in-tree library; otherwise (re)build it if its sources changed.
+    path = os.environ.get("SACRA_LIB") or _build.build()   # raises if nvcc fails: no silent fallback
+    lib = C.CDLL(path)
+    vp, dp, i32, i64 = C.c_void_p, C.c_void_p, C.c_int, C.c_int64
+    lib.sacra_fill_ghosts.argtypes = [vp, i32, dp, vp]
+    lib.sacra_z4c_rhs.argtypes = [vp, i32, vp, dp, dp, vp]
+    lib.sacra_rk4_substep.argtypes = [vp, i32, vp, i32, dp, dp, dp, dp, vp]
+    lib.sacra_rk4_step.argtypes = [vp, i32, vp, dp, dp, i64, vp]
+    for n in EXPORTS[:4]:
+        getattr(lib, n).restype = C.c_int
+    lib.sacra_strerror.argtypes = [C.c_int]
+    lib.sacra_strerror.restype = C.c_char_p
+    lib.sacra_version.restype = C.c_char_p
+    return lib, path
+
+
+lib, LIB_PATH = _load()
+
+
+def strerror(code: int) -> str:
+    return lib.sacra_strerror(int(code)).decode()
+
+
+def version() -> str:
+    return lib.sacra_version().decode()
+
+
+def make_patches(ps):
+    """list of objects with nx ny nz pitch_x field_stride patch_offset dx dt [ng] -> (SacraPatch*n)"""
+    if isinstance(ps, C.Array):
+        return ps
+    arr = (SacraPatch * len(ps))()
+    for a, p in zip(arr, ps):
+        a.nx, a.ny, a.nz, a.ng = p.nx, p.ny, p.nz, getattr(p, "ng", NG)
+        a.pitch_x, a.field_stride, a.patch_offset = p.pitch_x, p.field_stride, p.patch_offset
+        a.dx, a.dt = p.dx, p.dt
+    return arr
+
+
+def make_params(d):
+    if isinstance(d, SacraParams):
+        return d
+    return SacraParams(d["kappa1"], d["kappa2"], d["eta"], d["shift_coef"], d["ko_sigma"],
+                       int(d.get("lapse_uses_khat", 1)), 0)
+
+
+def _ptr(t):
+    """device pointer of a torch CUDA float64 tensor, or an int/None passed through"""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if not (t.is_cuda and t.dtype.is_floating_point and t.element_size() == 8 and t.is_contiguous()):
+        raise TypeError("libsacra takes contiguous CUDA float64 tensors")
+    return t.data_ptr()
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return stream if isinstance(stream, int) else stream.cuda_stream
+
+
+def _check(code):
+    if code != OK:
+        raise SacraError(code)
+
+
+def _ref(x):
+    return C.byref(x) if x is not None else None
+
+
+def fill_ghosts(patches, u, stream=None):
+    ps = make_patches(patches) if patches is not None else None
+    _check(lib.sacra_fill_ghosts(ps, len(ps) if ps is not None else 0, _ptr(u), _stream(stream)))
+
+
+def z4c_rhs(patches, params, u, rhs, stream=None):
+    ps = make_patches(patches) if patches is not None else None
+    pr = make_params(params) if params is not None else None
+    _check(lib.sacra_z4c_rhs(ps, len(ps) if ps is not None else 0, _ref(pr), _ptr(u), _ptr(rhs),
+                             _stream(stream)))
+
+
+def rk4_substep(patches, params, stage, u_n, u_in, u_out, acc, stream=None):
+    ps = make_patches(patches) if patches is not None else None
+    pr = make_params(params) if params is not None else None
+    _check(lib.sacra_rk4_substep(ps, len(ps) if ps is not None else 0, _ref(pr), int(stage), _ptr(u_n),
+                                 _ptr(u_in), _ptr(u_out), _ptr(acc), _stream(stream)))
+
+
+def rk4_step(patches, params, u, work, state_doubles=None, stream=None):
+    """work: one tensor of 3*state_doubles; state_doubles defaults to u.numel()."""
+    ps = make_patches(patches) if patches is not None else None
+    pr = make_params(params) if params is not None else None
+    if state_doubles is None:
+        state_doubles = u.numel()
+    _check(lib.sacra_rk4_step(ps, len(ps) if ps is not None else 0, _ref(pr), _ptr(u), _ptr(work),
+                              int(state_doubles), _stream(stream)))

@@ -154,11 +154,20 @@ def _flat_fields(shape):
 
 def _store(wl: Workload, ip: int, fields, seed, amp):
     p = wl.patches[ip]
-    for f in range(NF):
+
+    def one(f):
         a = np.array(fields[f], dtype=np.float64, copy=True)
         if amp:
             a = a + noise(seed, ip, f, p.nz, p.ny, p.nx, amp)
         wl.active_view(wl.state, ip, f)[...] = a
+
+    if p.npoints >= 1 << 21:           # large patches: fields in parallel (numpy releases the GIL)
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(max_workers=8) as ex:
+            list(ex.map(one, range(NF)))
+    else:
+        for f in range(NF):
+            one(f)
 
 
 def _puncture_fields(p: Patch, punctures, symmetric=False):

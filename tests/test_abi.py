@@ -1,0 +1,95 @@
+"""C ABI of libsacra (include/sacra.h): the library loads, exports every declared symbol, and rejects bad
+arguments before touching the GPU (SURVEY 8(b) error list). No compute calls: runs without a device."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2607_08743_b200 import sacra
+from paper_2607_08743_b200 import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+FAKE = 0x10000  # a non-null, 16-byte aligned "device pointer"; validation must fail before any launch
+
+
+def _declared():
+    txt = open(os.path.join(ROOT, "include", "sacra.h")).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(sacra_[a-z0-9_]+)\s*\(", txt)))
+
+
+def test_library_exports_every_declared_symbol():
+    names = _declared()
+    assert set(names) >= {"sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4_step",
+                          "sacra_strerror"}
+    lib = C.CDLL(sacra.LIB_PATH)
+    for n in names:
+        assert hasattr(lib, n), n
+    assert set(sacra.EXPORTS) == set(names)
+
+
+def test_struct_layout_matches_header():
+    assert C.sizeof(sacra.SacraPatch) == 4 * 4 + 3 * 8 + 2 * 8
+    assert C.sizeof(sacra.SacraParams) == 5 * 8 + 2 * 4
+    assert sacra.version()
+
+
+def test_strerror_covers_every_code():
+    seen = {sacra.strerror(c) for c in range(0, -6, -1)}
+    assert len(seen) == 6 and sacra.strerror(-99) not in seen
+
+
+def _patch(**kw):
+    ps, total = wl.make_layout([(8, 8, 8)], [0.1], [0.025], [(0, 0, 0)])
+    p = ps[0]
+    for k, v in kw.items():
+        setattr(p, k, v)
+    return [p], total
+
+
+def _code(fn, *a):
+    with pytest.raises(sacra.SacraError) as e:
+        fn(*a, stream=0)
+    return e.value.code
+
+
+PRM = dict(wl.DEFAULT_PARAMS)
+
+
+def test_null_pointers():
+    ps, _ = _patch()
+    assert _code(sacra.fill_ghosts, ps, None) == sacra.ERR_NULL
+    assert _code(sacra.fill_ghosts, None, FAKE) == sacra.ERR_NULL
+    assert _code(sacra.z4c_rhs, ps, None, FAKE, FAKE + 64) == sacra.ERR_NULL
+    assert _code(sacra.z4c_rhs, ps, PRM, None, FAKE) == sacra.ERR_NULL
+    assert _code(sacra.rk4_substep, ps, PRM, 1, FAKE, FAKE, None, FAKE + 64) == sacra.ERR_NULL
+    assert _code(sacra.rk4_step, ps, PRM, FAKE, None, 1024) == sacra.ERR_NULL
+
+
+def test_bad_arguments():
+    assert _code(sacra.fill_ghosts, _patch(ng=2)[0], FAKE) == sacra.ERR_UNSUPPORTED
+    assert _code(sacra.fill_ghosts, _patch(nx=5)[0], FAKE) == sacra.ERR_BADARG
+    assert _code(sacra.fill_ghosts, _patch(dx=0.0)[0], FAKE) == sacra.ERR_BADARG
+    assert _code(sacra.fill_ghosts, _patch(dx=float("nan"))[0], FAKE) == sacra.ERR_BADARG
+    assert _code(sacra.fill_ghosts, _patch(pitch_x=12)[0], FAKE) == sacra.ERR_BADARG      # < nx+6
+    assert _code(sacra.fill_ghosts, _patch(field_stride=100)[0], FAKE) == sacra.ERR_BADARG
+    assert _code(sacra.fill_ghosts, _patch(patch_offset=-3)[0], FAKE) == sacra.ERR_BADARG
+    assert _code(sacra.fill_ghosts, [], FAKE) == sacra.ERR_BADARG                          # npatch < 1
+    ps, total = _patch()
+    for stage in (0, 5, -1):
+        assert _code(sacra.rk4_substep, ps, PRM, stage, FAKE, FAKE + 64, FAKE + 128, FAKE + 192) == sacra.ERR_BADARG
+    # forbidden aliasing: u_out == u_in, acc == anything, rhs == u
+    assert _code(sacra.rk4_substep, ps, PRM, 2, FAKE, FAKE + 64, FAKE + 64, FAKE + 192) == sacra.ERR_BADARG
+    assert _code(sacra.rk4_substep, ps, PRM, 2, FAKE, FAKE + 64, FAKE + 128, FAKE) == sacra.ERR_BADARG
+    assert _code(sacra.z4c_rhs, ps, PRM, FAKE, FAKE) == sacra.ERR_BADARG
+    # state too small for the patch
+    assert _code(sacra.rk4_step, ps, PRM, FAKE, FAKE + 64, 1000) == sacra.ERR_BADARG
+
+
+def test_alignment():
+    ps, _ = _patch()
+    assert _code(sacra.fill_ghosts, ps, FAKE + 8) == sacra.ERR_ALIGN
+    assert _code(sacra.fill_ghosts, _patch(pitch_x=15)[0], FAKE) == sacra.ERR_ALIGN
+    assert _code(sacra.fill_ghosts, _patch(patch_offset=4)[0], FAKE) == sacra.ERR_ALIGN    # offset+ng odd
+    assert _code(sacra.z4c_rhs, ps, PRM, FAKE, FAKE + 8) == sacra.ERR_ALIGN
