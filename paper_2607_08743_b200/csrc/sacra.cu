@@ -10,7 +10,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/sacra.h"
-#include "z4c_point.cuh"
+#include "z4c_fused.cuh"
 
 namespace sacra {
 
@@ -65,66 +65,26 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Derivative stage, direct from global memory through L1/L2 (version 1: no staging).
+// Fused substage kernel: one thread per active point; samples come straight from global memory
+// through L1/L2 (blocks are 3-D tiles so that most stencil neighbours hit L1).
 // ---------------------------------------------------------------------------------------------------
-template <int F>
-__device__ __forceinline__ void derivs_of_field(const double* __restrict__ c, long long sy, long long sz,
-                                                const Coef& cf, const double (&beta)[3],
-                                                const double (&sg)[3], Derivs& D, double& u0_out) {
-  const long long st[3] = {1, sy, sz};
-  const double u0 = __ldg(c);
-  u0_out = u0;
-  double qsum = 0.0, adv[3];
-#pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    const long long s = st[a];
-    const double m3 = __ldg(c - 3 * s), m2 = __ldg(c - 2 * s), m1 = __ldg(c - s);
-    const double p1 = __ldg(c + s), p2 = __ldg(c + 2 * s), p3 = __ldg(c + 3 * s);
-    if (d1slot(F) >= 0) D.d1[d1slot(F)][a] = __dmul_rn(d1_num(m2, m1, p1, p2), cf.inv12h);
-    const double s1 = pair_sum(m1, u0, p1), s2 = pair_sum(m2, u0, p2), s3 = pair_sum(m3, u0, p3);
-    if (d2slot(F) >= 0) D.d2[d2slot(F)][sym(a, a)] = __dmul_rn(d2_num(s1, s2), cf.inv12h2);
-    const double q = ko_num(s1, s2, s3);
-    qsum = (a == 0) ? q : __dadd_rn(qsum, q);
-    // upwind: v_k = u(x + sg k h); select mirrored samples by the sign of beta^a (same instructions for
-    // both signs: item 13)
-    const bool pos = sg[a] > 0.0;
-    const double vm1 = pos ? m1 : p1, v1 = pos ? p1 : m1, v2 = pos ? p2 : m2, v3 = pos ? p3 : m3;
-    adv[a] = __dmul_rn(beta[a], __dmul_rn(up_num(vm1, u0, v1, v2, v3, sg[a]), cf.inv12h));
-  }
-  D.adv[F] = __dadd_rn(__dadd_rn(adv[0], adv[1]), adv[2]);
-  D.ko[F] = __dmul_rn(qsum, cf.kofac);
-  if (d2slot(F) >= 0) {
-    // mixed second derivatives D_ab = D_a(D_b u), a < b, inner (unscaled) difference along the later axis b
-#pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-      for (int b = a + 1; b < 3; ++b) {
-        const long long sa = st[a], sb = st[b];
-        auto e = [&](long long o) {
-          const double* v = c + o;
-          return d1_num(__ldg(v - 2 * sb), __ldg(v - sb), __ldg(v + sb), __ldg(v + 2 * sb));
-        };
-        const double em2 = e(-2 * sa), em1 = e(-sa), ep1 = e(sa), ep2 = e(2 * sa);
-        D.d2[d2slot(F)][sym(a, b)] = __dmul_rn(d1_num(em2, em1, ep1, ep2), cf.inv144h2);
-      }
-  }
-}
+constexpr int TX = 32, TY = 4, TZ = 2;       // tile = thread block
 
-template <int F>
-struct FieldLoop {
-  static __device__ __forceinline__ void run(const double* __restrict__ base, long long fstride, long long c,
-                                             long long sy, long long sz, const Coef& cf,
-                                             const double (&beta)[3], const double (&sg)[3], Derivs& D,
-                                             double (&u)[NF]) {
-    derivs_of_field<F>(base + (long long)F * fstride + c, sy, sz, cf, beta, sg, D, u[F]);
-    FieldLoop<F + 1>::run(base, fstride, c, sy, sz, cf, beta, sg, D, u);
+struct GlobalLoader {      // sample loader of one field for field_derivs()
+  const double* c;         // centre
+  long long st[3];         // strides along x, y, z in doubles
+  __device__ __forceinline__ double operator()(int a, int k) const { return __ldg(c + k * st[a]); }
+  __device__ __forceinline__ double mixed(int a, int ka, int b, int kb) const {
+    return __ldg(c + ka * st[a] + kb * st[b]);
   }
 };
-template <>
-struct FieldLoop<NF> {
-  static __device__ __forceinline__ void run(const double* __restrict__, long long, long long, long long,
-                                             long long, const Coef&, const double (&)[3], const double (&)[3],
-                                             Derivs&, double (&)[NF]) {}
+struct GlobalSource {
+  const double* base;      // field 0 at the centre point
+  long long fstride, sy, sz;
+  template <int F> __device__ __forceinline__ GlobalLoader field() const {
+    return GlobalLoader{base + (long long)F * fstride, {1, sy, sz}};
+  }
+  __device__ __forceinline__ double centre(int f) const { return __ldg(base + (long long)f * fstride); }
 };
 
 // EPI: 0 = store RHS; 1..4 = RK4 substage (item 11 table)
@@ -135,63 +95,56 @@ struct RkArgs {
 };
 
 template <int EPI>
-__global__ void __launch_bounds__(128) k_z4c(const __grid_constant__ PatchBatch B, const __grid_constant__ Params P,
-                                             const double* __restrict__ u_in, double* __restrict__ rhs,
-                                             const __grid_constant__ RkArgs rk) {
+struct Emitter {
+  double* rhs;             // EPI == 0
+  RkArgs rk;
+  long long o, fstride;    // offset of field 0 at this point, field stride
+  double dt;
+  __device__ __forceinline__ void operator()(int f, double kk) const {
+    const long long a = o + (long long)f * fstride;
+    if (EPI == 0) { rhs[a] = kk; return; }
+    const double un = rk.u_n[a];
+    if (EPI == 1) {
+      rk.acc[a] = kk;
+      rk.u_out[a] = __dadd_rn(un, __dmul_rn(dt / 2.0, kk));
+    } else if (EPI == 2) {
+      rk.acc[a] = __dadd_rn(rk.acc[a], __dmul_rn(2.0, kk));
+      rk.u_out[a] = __dadd_rn(un, __dmul_rn(dt / 2.0, kk));
+    } else if (EPI == 3) {
+      rk.acc[a] = __dadd_rn(rk.acc[a], __dmul_rn(2.0, kk));
+      rk.u_out[a] = __dadd_rn(un, __dmul_rn(dt, kk));
+    } else {
+      const double S = __dmul_rn(__dadd_rn(rk.acc[a], kk), 1.0 / 6.0);
+      rk.acc[a] = S;
+      rk.u_out[a] = __dadd_rn(un, __dmul_rn(dt, S));
+    }
+  }
+};
+
+template <int EPI>
+__global__ void __launch_bounds__(TX * TY * TZ) k_z4c(const __grid_constant__ PatchBatch B,
+                                                      const __grid_constant__ Params P,
+                                                      const double* __restrict__ u_in, double* __restrict__ rhs,
+                                                      const __grid_constant__ RkArgs rk) {
   int ip = 0;
 #pragma unroll 1
   while (ip + 1 < B.np && (int)blockIdx.x >= B.first_block[ip + 1]) ++ip;
   const DevPatch& p = B.p[ip];
-  // block -> (x-chunk, j-chunk, k) ; blockDim = (32, 4)
-  const int nbx = (p.nx + 31) / 32, nby = (p.ny + 3) / 4;
+  const int nbx = (p.nx + TX - 1) / TX, nby = (p.ny + TY - 1) / TY;
   int b = (int)blockIdx.x - B.first_block[ip];
   const int bx = b % nbx; b /= nbx;
-  const int by = b % nby; const int k = b / nby;
-  const int i = bx * 32 + threadIdx.x, j = by * 4 + threadIdx.y;
-  if (i >= p.nx || j >= p.ny) return;
+  const int by = b % nby; const int bz = b / nby;
+  const int i = bx * TX + threadIdx.x, j = by * TY + threadIdx.y, k = bz * TZ + threadIdx.z;
+  if (i >= p.nx || j >= p.ny || k >= p.nz) return;
   const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
-  const double* base = u_in + p.offset;
-
-  const Coef cf = make_coef(p.dx, P.ko_sigma);
-  double beta[3], sg[3];
+  const GlobalSource src{u_in + p.offset + c, p.fstride, p.pitch, p.sz};
+  double beta[3];
 #pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    beta[a] = __ldg(base + (long long)(F_BET + a) * p.fstride + c);
-    sg[a] = beta[a] >= 0.0 ? 1.0 : -1.0;
-  }
-  Derivs D;
-  double u[NF], out[NF];
-  FieldLoop<0>::run(base, p.fstride, c, p.pitch, p.sz, cf, beta, sg, D, u);
-  z4c_algebra(u, D, P, out);
-
-  const long long o = p.offset + c;
-  if (EPI == 0) {
-#pragma unroll
-    for (int f = 0; f < NF; ++f) rhs[o + (long long)f * p.fstride] = out[f];
-  } else {
-    const double dt = p.dt;
-    const double hdt = dt / 2.0, c6 = 1.0 / 6.0;
-#pragma unroll
-    for (int f = 0; f < NF; ++f) {
-      const long long a = o + (long long)f * p.fstride;
-      const double kk = out[f];
-      const double un = rk.u_n[a];
-      if (EPI == 1) {
-        rk.acc[a] = kk;
-        rk.u_out[a] = __dadd_rn(un, __dmul_rn(hdt, kk));
-      } else if (EPI == 2) {
-        rk.acc[a] = __dadd_rn(rk.acc[a], __dmul_rn(2.0, kk));
-        rk.u_out[a] = __dadd_rn(un, __dmul_rn(hdt, kk));
-      } else if (EPI == 3) {
-        rk.acc[a] = __dadd_rn(rk.acc[a], __dmul_rn(2.0, kk));
-        rk.u_out[a] = __dadd_rn(un, __dmul_rn(dt, kk));
-      } else {
-        const double S = __dmul_rn(__dadd_rn(rk.acc[a], kk), c6);
-        rk.acc[a] = S;
-        rk.u_out[a] = __dadd_rn(un, __dmul_rn(dt, S));
-      }
-    }
-  }
+  for (int a = 0; a < 3; ++a) beta[a] = src.centre(F_BET + a);
+  PointCoef pc;
+  make_coef(p.dx, P.ko_sigma, beta, pc);
+  Emitter<EPI> emit{rhs, rk, p.offset + c, p.fstride, p.dt};
+  z4c_point(src, P, pc, emit);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -260,10 +213,10 @@ static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* 
     for (int q = 0; q < B.np; ++q) {
       B.p[q] = to_dev(p[q0 + q]);
       B.first_block[q] = nb;
-      nb += ((p[q0 + q].nx + 31) / 32) * ((p[q0 + q].ny + 3) / 4) * p[q0 + q].nz;
+      nb += ((p[q0 + q].nx + TX - 1) / TX) * ((p[q0 + q].ny + TY - 1) / TY) * ((p[q0 + q].nz + TZ - 1) / TZ);
     }
     B.first_block[B.np] = nb;
-    const dim3 blk(32, 4);
+    const dim3 blk(TX, TY, TZ);
     switch (epi) {
       case 0: k_z4c<0><<<nb, blk, 0, st>>>(B, P, u_in, rhs, rk); break;
       case 1: k_z4c<1><<<nb, blk, 0, st>>>(B, P, u_in, rhs, rk); break;
