@@ -11,6 +11,7 @@
 
 #include "../../include/sacra.h"
 #include "z4c_fused.cuh"
+#include "z4c_tile.cuh"
 
 namespace sacra {
 
@@ -65,26 +66,13 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Fused substage kernel: one thread per active point; samples come straight from global memory
-// through L1/L2 (blocks are 3-D tiles so that most stencil neighbours hit L1).
+// Fused substage kernel: persistent CTAs, one thread per active point of a TX x TY x TZ tile; the 25 fields
+// are streamed through a TMA ring in shared memory (z4c_tile.cuh).
 // ---------------------------------------------------------------------------------------------------
-constexpr int TX = 32, TY = 4, TZ = 2;       // tile = thread block
+using Tile = TileCfg<16, 4, 4, 5>;
 
-struct GlobalLoader {      // sample loader of one field for field_derivs()
-  const double* c;         // centre
-  long long st[3];         // strides along x, y, z in doubles
-  __device__ __forceinline__ double operator()(int a, int k) const { return __ldg(c + k * st[a]); }
-  __device__ __forceinline__ double mixed(int a, int ka, int b, int kb) const {
-    return __ldg(c + ka * st[a] + kb * st[b]);
-  }
-};
-struct GlobalSource {
-  const double* base;      // field 0 at the centre point
-  long long fstride, sy, sz;
-  template <int F> __device__ __forceinline__ GlobalLoader field() const {
-    return GlobalLoader{base + (long long)F * fstride, {1, sy, sz}};
-  }
-  __device__ __forceinline__ double centre(int f) const { return __ldg(base + (long long)f * fstride); }
+struct alignas(64) TileMaps {   // one rank-4 (x, y, z, field) tensor map per patch of the launch
+  CUtensorMap m[MAXP];
 };
 
 // EPI: 0 = store RHS; 1..4 = RK4 substage (item 11 table)
@@ -94,13 +82,17 @@ struct RkArgs {
   double* acc;
 };
 
+// active: out-of-range threads of a ragged tile run the same instruction stream on clamped / zero-filled data
+// (they must reach every barrier) and store nothing.
 template <int EPI>
 struct Emitter {
   double* rhs;             // EPI == 0
   RkArgs rk;
   long long o, fstride;    // offset of field 0 at this point, field stride
   double dt;
+  bool active;
   __device__ __forceinline__ void operator()(int f, double kk) const {
+    if (!active) return;
     const long long a = o + (long long)f * fstride;
     if (EPI == 0) { rhs[a] = kk; return; }
     const double un = rk.u_n[a];
@@ -121,30 +113,88 @@ struct Emitter {
   }
 };
 
-template <int EPI>
-__global__ void __launch_bounds__(TX * TY * TZ) k_z4c(const __grid_constant__ PatchBatch B,
-                                                      const __grid_constant__ Params P,
-                                                      const double* __restrict__ u_in, double* __restrict__ rhs,
-                                                      const __grid_constant__ RkArgs rk) {
-  int ip = 0;
+struct TileId {   // a tile of the launch: patch and tile indices
+  int ip, bx, by, bz;
+};
+template <class C>
+__device__ __forceinline__ TileId locate(const PatchBatch& B, int t) {
+  TileId id;
+  id.ip = 0;
 #pragma unroll 1
-  while (ip + 1 < B.np && (int)blockIdx.x >= B.first_block[ip + 1]) ++ip;
-  const DevPatch& p = B.p[ip];
-  const int nbx = (p.nx + TX - 1) / TX, nby = (p.ny + TY - 1) / TY;
-  int b = (int)blockIdx.x - B.first_block[ip];
-  const int bx = b % nbx; b /= nbx;
-  const int by = b % nby; const int bz = b / nby;
-  const int i = bx * TX + threadIdx.x, j = by * TY + threadIdx.y, k = bz * TZ + threadIdx.z;
-  if (i >= p.nx || j >= p.ny || k >= p.nz) return;
-  const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
-  const GlobalSource src{u_in + p.offset + c, p.fstride, p.pitch, p.sz};
-  double beta[3];
+  while (id.ip + 1 < B.np && t >= B.first_block[id.ip + 1]) ++id.ip;
+  const DevPatch& p = B.p[id.ip];
+  const int nbx = (p.nx + C::TX - 1) / C::TX, nby = (p.ny + C::TY - 1) / C::TY;
+  int b = t - B.first_block[id.ip];
+  id.bx = b % nbx; b /= nbx;
+  id.by = b % nby; id.bz = b / nby;
+  return id;
+}
+
+template <int EPI>
+__global__ void __launch_bounds__(Tile::NT, 1) k_z4c(const __grid_constant__ PatchBatch B,
+                                                     const __grid_constant__ Params P,
+                                                     const __grid_constant__ TileMaps M,
+                                                     const double* __restrict__ u_in, double* __restrict__ rhs,
+                                                     const __grid_constant__ RkArgs rk) {
+  using C = Tile;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double* ring = reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+  uint64_t* full = reinterpret_cast<uint64_t*>(ring + C::NS * C::SLOT);
+  const int ntiles = B.first_block[B.np];
+  const bool leader = (threadIdx.x | threadIdx.y | threadIdx.z) == 0;
+
+  int t = blockIdx.x;
+  if (t >= ntiles) return;
+  TileId id = locate<C>(B, t);
+  // tensor-map x coordinate c <-> storage cell c-1 (the map starts one double before storage cell 0, on a
+  // 16-byte boundary); the box of tile bx starts at the even coordinate bx*TX = storage cell bx*TX - 1
+  TileSource<C> src;
+  src.cur = TileCoord{&M.m[id.ip], id.bx * C::TX, id.by * C::TY, id.bz * C::TZ};
+  if (leader) {
+    for (int s = 0; s < C::NS; ++s) tma::mbar_init(full + s, 1);
+    tma::fence_mbar_init();
+  }
+  __syncthreads();
+  if (leader) {   // prime the ring with the first NS-1 fields of the first tile
+    if (C::NS > 1) TileSource<C>::template issue<0>(ring, full, src.cur);
+    if (C::NS > 2) TileSource<C>::template issue<1 % NF>(ring, full, src.cur);
+    if (C::NS > 3) TileSource<C>::template issue<2 % NF>(ring, full, src.cur);
+    if (C::NS > 4) TileSource<C>::template issue<3 % NF>(ring, full, src.cur);
+    static_assert(C::NS <= 5, "prime more fields");
+  }
+  src.ring = ring;
+  src.full = full;
+  src.sc = ring + ((threadIdx.z + NG) * C::PY + (threadIdx.y + NG)) * C::PX + (threadIdx.x + C::XC);
+
+#pragma unroll 1
+  for (uint32_t iter = 0;; ++iter) {
+    const DevPatch& p = B.p[id.ip];
+    const int tn = t + gridDim.x;
+    src.has_next = tn < ntiles;
+    TileId idn = id;
+    if (src.has_next) {
+      idn = locate<C>(B, tn);
+      src.nxt = TileCoord{&M.m[idn.ip], idn.bx * C::TX, idn.by * C::TY, idn.bz * C::TZ};
+    }
+    src.iter = iter;
+    const int i = id.bx * C::TX + threadIdx.x, j = id.by * C::TY + threadIdx.y, k = id.bz * C::TZ + threadIdx.z;
+    const bool active = (i < p.nx) & (j < p.ny) & (k < p.nz);
+    const int ic = min(i, p.nx - 1), jc = min(j, p.ny - 1), kc = min(k, p.nz - 1);
+    const long long c = (long long)(kc + NG) * p.sz + (long long)(jc + NG) * p.pitch + (ic + NG);
+    src.gcentre = u_in + p.offset + c;
+    src.fstride = p.fstride;
+    double beta[3];
 #pragma unroll
-  for (int a = 0; a < 3; ++a) beta[a] = src.centre(F_BET + a);
-  PointCoef pc;
-  make_coef(p.dx, P.ko_sigma, beta, pc);
-  Emitter<EPI> emit{rhs, rk, p.offset + c, p.fstride, p.dt};
-  z4c_point(src, P, pc, emit);
+    for (int a = 0; a < 3; ++a) beta[a] = src.centre(F_BET + a);
+    PointCoef pc;
+    make_coef(p.dx, P.ko_sigma, beta, pc);
+    Emitter<EPI> emit{rhs, rk, p.offset + c, p.fstride, p.dt, active};
+    z4c_point(src, P, pc, emit);
+    if (!src.has_next) break;
+    t = tn;
+    id = idn;
+    src.cur = src.nxt;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -201,30 +251,90 @@ static int launch_fill(const sacra_patch_t* p, int npatch, double* u, cudaStream
   return SACRA_OK;
 }
 
+// cuTensorMapEncodeTiled through the runtime (libsacra does not link libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled() {
+  static EncodeTiledFn fn = [] {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      f = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(f);
+  }();
+  return fn;
+}
+
+// Rank-4 (x, y, z, field) map of one patch of state `u`. Storage cell 0 of a row sits at an odd double
+// (sacra.h: active cell 0 is 16-byte aligned and ng = 3), so the map starts ONE double earlier, which is
+// 16-byte aligned and inside the caller's buffer (patch_offset >= 1); kernel x coordinates are shifted by +1.
+static int make_map(const sacra_patch_t& a, const double* u, CUtensorMap* out) {
+  EncodeTiledFn enc = encode_tiled();
+  if (!enc) return SACRA_ERR_CUDA;
+  const cuuint64_t dims[4] = {(cuuint64_t)a.nx + 2 * NG + 1, (cuuint64_t)a.ny + 2 * NG, (cuuint64_t)a.nz + 2 * NG, NF};
+  const cuuint64_t strides[3] = {(cuuint64_t)a.pitch_x * 8, (cuuint64_t)a.pitch_x * (a.ny + 2 * NG) * 8,
+                                 (cuuint64_t)a.field_stride * 8};
+  const cuuint32_t box[4] = {Tile::PX, Tile::PY, Tile::PZ, 1};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  void* base = const_cast<double*>(u + a.patch_offset - 1);
+  const CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? SACRA_OK : SACRA_ERR_CUDA;
+}
+
+static int num_sms() {
+  static int n = [] {
+    int dev = 0, v = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+    return v;
+  }();
+  return n;
+}
+
+template <int EPI>
+static cudaError_t launch_one(int grid, cudaStream_t st, const PatchBatch& B, const Params& P, const TileMaps& M,
+                              const double* u_in, double* rhs, const RkArgs& rk) {
+  static const cudaError_t attr =
+      cudaFuncSetAttribute(k_z4c<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile::SMEM_BYTES);
+  if (attr != cudaSuccess) return attr;
+  k_z4c<EPI><<<grid, dim3(Tile::TX, Tile::TY, Tile::TZ), Tile::SMEM_BYTES, st>>>(B, P, M, u_in, rhs, rk);
+  return cudaGetLastError();
+}
+
 static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, int epi,
                       const double* u_in, double* rhs, const double* u_n, double* u_out, double* acc,
                       cudaStream_t st) {
   const Params P = to_dev(*prm);
   RkArgs rk{u_n, u_out, acc};
+  const int sms = num_sms();
+  if (sms <= 0) return SACRA_ERR_CUDA;
   for (int q0 = 0; q0 < npatch; q0 += MAXP) {
     PatchBatch B;
+    TileMaps M;
     B.np = (npatch - q0 < MAXP) ? npatch - q0 : MAXP;
     int nb = 0;
     for (int q = 0; q < B.np; ++q) {
-      B.p[q] = to_dev(p[q0 + q]);
+      const sacra_patch_t& a = p[q0 + q];
+      B.p[q] = to_dev(a);
       B.first_block[q] = nb;
-      nb += ((p[q0 + q].nx + TX - 1) / TX) * ((p[q0 + q].ny + TY - 1) / TY) * ((p[q0 + q].nz + TZ - 1) / TZ);
+      nb += ((a.nx + Tile::TX - 1) / Tile::TX) * ((a.ny + Tile::TY - 1) / Tile::TY) * ((a.nz + Tile::TZ - 1) / Tile::TZ);
+      if (int e = make_map(a, u_in, &M.m[q])) return e;
     }
     B.first_block[B.np] = nb;
-    const dim3 blk(TX, TY, TZ);
+    const int grid = nb < sms ? nb : sms;   // persistent: one CTA per SM, tiles dealt round-robin
+    cudaError_t err;
     switch (epi) {
-      case 0: k_z4c<0><<<nb, blk, 0, st>>>(B, P, u_in, rhs, rk); break;
-      case 1: k_z4c<1><<<nb, blk, 0, st>>>(B, P, u_in, rhs, rk); break;
-      case 2: k_z4c<2><<<nb, blk, 0, st>>>(B, P, u_in, rhs, rk); break;
-      case 3: k_z4c<3><<<nb, blk, 0, st>>>(B, P, u_in, rhs, rk); break;
-      default: k_z4c<4><<<nb, blk, 0, st>>>(B, P, u_in, rhs, rk); break;
+      case 0: err = launch_one<0>(grid, st, B, P, M, u_in, rhs, rk); break;
+      case 1: err = launch_one<1>(grid, st, B, P, M, u_in, rhs, rk); break;
+      case 2: err = launch_one<2>(grid, st, B, P, M, u_in, rhs, rk); break;
+      case 3: err = launch_one<3>(grid, st, B, P, M, u_in, rhs, rk); break;
+      default: err = launch_one<4>(grid, st, B, P, M, u_in, rhs, rk); break;
     }
-    if (cudaGetLastError() != cudaSuccess) return SACRA_ERR_CUDA;
+    if (err != cudaSuccess) return SACRA_ERR_CUDA;
   }
   return SACRA_OK;
 }
