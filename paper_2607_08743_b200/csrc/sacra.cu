@@ -137,9 +137,6 @@ __global__ void __launch_bounds__(Tile::NT, 1) k_z4c(const __grid_constant__ Pat
                                                      const double* __restrict__ u_in, double* __restrict__ rhs,
                                                      const __grid_constant__ RkArgs rk) {
   using C = Tile;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  double* ring = reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
-  uint64_t* full = reinterpret_cast<uint64_t*>(ring + C::NS * C::SLOT);
   const int ntiles = B.first_block[B.np];
   const bool leader = (threadIdx.x | threadIdx.y | threadIdx.z) == 0;
 
@@ -151,20 +148,21 @@ __global__ void __launch_bounds__(Tile::NT, 1) k_z4c(const __grid_constant__ Pat
   TileSource<C> src;
   src.cur = TileCoord{&M.m[id.ip], id.bx * C::TX, id.by * C::TY, id.bz * C::TZ};
   if (leader) {
-    for (int s = 0; s < C::NS; ++s) tma::mbar_init(full + s, 1);
+    for (int s = 0; s < C::NS; ++s) tma::mbar_init(TileSource<C>::full(s), 1);
     tma::fence_mbar_init();
   }
   __syncthreads();
   if (leader) {   // prime the ring with the first NS-1 fields of the first tile
-    if (C::NS > 1) TileSource<C>::template issue<0>(ring, full, src.cur);
-    if (C::NS > 2) TileSource<C>::template issue<1 % NF>(ring, full, src.cur);
-    if (C::NS > 3) TileSource<C>::template issue<2 % NF>(ring, full, src.cur);
-    if (C::NS > 4) TileSource<C>::template issue<3 % NF>(ring, full, src.cur);
+    if (C::NS > 1) TileSource<C>::template issue<0>(src.cur);
+    if (C::NS > 2) TileSource<C>::template issue<1 % NF>(src.cur);
+    if (C::NS > 3) TileSource<C>::template issue<2 % NF>(src.cur);
+    if (C::NS > 4) TileSource<C>::template issue<3 % NF>(src.cur);
     static_assert(C::NS <= 5, "prime more fields");
   }
-  src.ring = ring;
-  src.full = full;
-  src.sc = ring + ((threadIdx.z + NG) * C::PY + (threadIdx.y + NG)) * C::PX + (threadIdx.x + C::XC);
+  build_e_table<C>();   // visible after the first barrier of field<>()
+  src.ey = C::EY_OFF + (threadIdx.z * C::TY + threadIdx.y) * C::EX + (threadIdx.x + 2);
+  src.ez = C::EZ_OFF + (threadIdx.z * (C::TY + 4) + (threadIdx.y + 2)) * C::EX + (threadIdx.x + 2);
+  src.sc = ((threadIdx.z + NG) * C::PY + (threadIdx.y + NG)) * C::PX + (threadIdx.x + C::XC);
 
 #pragma unroll 1
   for (uint32_t iter = 0;; ++iter) {

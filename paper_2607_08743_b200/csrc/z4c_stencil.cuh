@@ -3,12 +3,14 @@
 // SURVEY 8(c) items 3-6 (4th-order centred differences, 4th-order upwind along the shift,
 // Kreiss-Oliger dissipation), all in DIFFERENCE FORM: the first operation on any sample is a subtraction
 // of a neighbouring sample, so round-off scales with the field's variation, not its magnitude.
-//   * every operator is evaluated in the canonical operation order of SURVEY 8(c) items 3-6, one rounding per
-//     written operation (the library is built with -fmad=false). The only FMAs are 8a-b and
-//     16p1-p2, where the product is exact, so the fused and unfused results are bit-identical.
-//   * the upwind side is chosen by SELECTING mirrored differences, never by branching: both signs of the
-//     shift execute the same instruction stream on mirrored data (bitwise pi-symmetry).
-// `Ld` is any callable sample loader: ld(a, k) = u(x + k h e_a), ld2(a, ka, b, kb) = u(x + ka h e_a + kb h e_b).
+//   * the centred first and second derivatives are evaluated in the canonical operation order of SURVEY 8(c)
+//     items 3-4 (the library is built with -fmad=false; the FMAs 8a-b and 16p1-p2 have an exact
+//     product, so they are bit-identical to the unfused form): D1, D_aa, D_ab are bit-identical to the oracle.
+//   * KO and the upwind stencil use explicit FMA chains (one rounding fewer per term than the oracle).
+//   * no data-dependent branch or select anywhere: both signs of the shift execute the same instruction
+//     stream on mirrored data (bitwise pi-symmetry).
+// `Ld` is the sample loader of one field: ld(a, k) = u(x + k h e_a); publish_e / e_y_x / e_z_x / e_z_y exchange the
+// inner first differences of the mixed second derivatives between the threads of a tile (z4c_tile.cuh).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -28,8 +30,8 @@ struct PointCoef {      // per-thread constants of the derivative stage
   double inv12h2;       // 1/(12 h^2)
   double inv144h2;      // 1/(144 h^2)
   double kofac;         // sigma/(64 h)
-  double beta[3];       // shift at the point
-  bool pos[3];          // beta^a >= 0 (reading I: the tie goes to +)
+  double ba[3];         // beta^a / (24 h)    weight of the antisymmetric part of the upwind stencil
+  double bs[3];         // |beta^a| / (24 h)  weight of its symmetric part
 };
 
 __device__ __forceinline__ void make_coef(double h, double sigma, const double (&beta)[3], PointCoef& c) {
@@ -37,10 +39,11 @@ __device__ __forceinline__ void make_coef(double h, double sigma, const double (
   c.inv12h2 = 1.0 / ((12.0 * h) * h);
   c.inv144h2 = 1.0 / ((144.0 * h) * h);
   c.kofac = sigma / (64.0 * h);
+  const double inv24h = 1.0 / (24.0 * h);
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
-    c.pos[a] = beta[a] >= 0.0;
-    c.beta[a] = beta[a];
+    c.ba[a] = beta[a] * inv24h;
+    c.bs[a] = fabs(beta[a]) * inv24h;
   }
 }
 
@@ -57,46 +60,47 @@ __device__ __forceinline__ double d1_num(double um2, double um1, double up1, dou
   return fma(8.0, up1 - um1, -(up2 - um2));
 }
 
+// Upwind advection without a data-dependent choice of samples. With v_k = u(x + sg k h), sg = sign(beta^a)
+// (the tie beta^a = 0 is immaterial: the term is multiplied by 0), the lopsided stencil of item 5 splits
+// exactly into an antisymmetric and a symmetric part,
+//   beta Dup u = beta [21 a1 - 6 a2 + a3] / (24 h)  +  |beta| [15 s1 - 6 s2 + s3] / (24 h),
+//   a_k = u(+k) - u(-k),   s_k = (u(+k) - u0) + (u(-k) - u0),
+// and the symmetric bracket IS the Kreiss-Oliger numerator q_a of item 6. Both signs of the shift run the same
+// instruction stream on mirrored data (bitwise pi-symmetry): under x -> -x, a_k -> -a_k
+// exactly, s_k -> s_k, beta -> -beta. a_k is one subtraction of two samples, so its round-off scales with the
+// field's variation like every other difference here. The oracle evaluates item 5 as written; the two agree
+// to a few ulp of the advection term.
 template <bool D1, bool D2, class Ld>
 __device__ __forceinline__ void field_derivs(const Ld& ld, const PointCoef& c, Stencil& S) {
+  static_assert(D1 || !D2, "the mixed second derivatives reuse the numerators of D_y, D_z");
   const double u0 = ld(0, 0);
   S.u0 = u0;
-  double adv[3], q = 0.0;
+  double adv = 0.0, q = 0.0, num[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     const double m3 = ld(a, -3), m2 = ld(a, -2), m1 = ld(a, -1);
     const double p1 = ld(a, 1), p2 = ld(a, 2), p3 = ld(a, 3);
-    if (D1) S.d1[a] = d1_num(m2, m1, p1, p2) * c.inv12h;
-    // differences to the centre, shared by D_aa, KO and the upwind stencil
-    const double dm1 = m1 - u0, dm2 = m2 - u0, dm3 = m3 - u0;
-    const double dp1 = p1 - u0, dp2 = p2 - u0, dp3 = p3 - u0;
-    const double s1 = dp1 + dm1, s2 = dp2 + dm2, s3 = dp3 + dm3;      // mirror-pair sums
-    if (D2) S.d2[sym(a, a)] = fma(16.0, s1, -s2) * c.inv12h2;         // item 4, diagonal
-    const double qa = (s3 - 6.0 * s2) + 15.0 * s1;                    // item 6: (p3 - 6 p2) + 15 p1
+    const double a1 = p1 - m1, a2 = p2 - m2, a3 = p3 - m3;            // antisymmetric differences
+    if (D1) {
+      num[a] = fma(8.0, a1, -a2);                                     // item 3 (8 a1 is exact)
+      S.d1[a] = num[a] * c.inv12h;
+    }
+    // differences to the centre, shared by D_aa, KO and the symmetric part of the upwind stencil
+    const double s1 = (p1 - u0) + (m1 - u0), s2 = (p2 - u0) + (m2 - u0), s3 = (p3 - u0) + (m3 - u0);
+    if (D2) S.d2[sym(a, a)] = fma(16.0, s1, -s2) * c.inv12h2;         // item 4, diagonal (16 s1 is exact)
+    const double qa = fma(15.0, s1, fma(-6.0, s2, s3));               // item 6: s3 - 6 s2 + 15 s1
     q = (a == 0) ? qa : q + qa;
-    // item 5: v_k = u(x + sg k h); numerator ((18 (v1-v0) - 3 (v-1-v0)) - 6 (v2-v0)) + (v3-v0)
-    const bool ps = c.pos[a];
-    const double w1 = ps ? dp1 : dm1, wm = ps ? dm1 : dp1, w2 = ps ? dp2 : dm2, w3 = ps ? dp3 : dm3;
-    const double r = ((18.0 * w1 - 3.0 * wm) - 6.0 * w2) + w3;
-    adv[a] = c.beta[a] * ((ps ? r : -r) * c.inv12h);                  // beta^a * ((sg r) / (12 h))
+    const double aa = fma(21.0, a1, fma(-6.0, a2, a3));               // item 5, antisymmetric bracket
+    adv = (a == 0) ? fma(c.bs[0], qa, c.ba[0] * aa) : fma(c.bs[a], qa, fma(c.ba[a], aa, adv));
   }
-  S.adv = (adv[0] + adv[1]) + adv[2];
+  S.adv = adv;
   S.ko = q * c.kofac;
   if (D2) {
-    // item 4, mixed: D_ab = D_a(D_b u), a < b, inner unscaled difference along the later axis b
-#pragma unroll
-    for (int a = 0; a < 3; ++a)
-#pragma unroll
-      for (int b = a + 1; b < 3; ++b) {
-        double e[4];
-#pragma unroll
-        for (int t = 0; t < 4; ++t) {
-          const int ka = (t < 2) ? t - 2 : t - 1;   // -2 -1 +1 +2
-          e[t] = d1_num(ld.mixed(a, ka, b, -2), ld.mixed(a, ka, b, -1), ld.mixed(a, ka, b, 1),
-                        ld.mixed(a, ka, b, 2));
-        }
-        S.d2[sym(a, b)] = d1_num(e[0], e[1], e[2], e[3]) * c.inv144h2;
-      }
+    // item 4, mixed: D_ab = D_a(e_b), a < b, e_b = unscaled inner difference along the later axis b
+    ld.publish_e(num[1], num[2]);
+    S.d2[sym(0, 1)] = d1_num(ld.e_y_x(-2), ld.e_y_x(-1), ld.e_y_x(1), ld.e_y_x(2)) * c.inv144h2;
+    S.d2[sym(0, 2)] = d1_num(ld.e_z_x(-2), ld.e_z_x(-1), ld.e_z_x(1), ld.e_z_x(2)) * c.inv144h2;
+    S.d2[sym(1, 2)] = d1_num(ld.e_z_y(-2), ld.e_z_y(-1), ld.e_z_y(1), ld.e_z_y(2)) * c.inv144h2;
   }
 }
 

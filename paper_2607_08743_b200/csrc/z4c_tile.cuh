@@ -73,22 +73,86 @@ struct TileCfg {
   static constexpr int BOX = PX * PY * PZ;                     // doubles per box
   static constexpr int BOX_BYTES = BOX * 8;
   static constexpr int SLOT = (BOX + 15) / 16 * 16;            // doubles per ring slot (128-byte multiple)
-  static constexpr int SMEM_BYTES = NS * SLOT * 8 + NS * 8 + 128;
+  // shared-memory map (in doubles): ring | mbarriers | E_y | E_z | halo-item table
+  static constexpr int BAR_OFF = NS * SLOT;                    // NS mbarriers (8 slots reserved)
+  static constexpr int EX = TX + 4;                            // x extent of the e arrays (x halo of 2)
+  static constexpr int EY_OFF = BAR_OFF + 8;                   // e_y on  TZ x TY x (TX+4)
+  static constexpr int EZ_OFF = EY_OFF + TZ * TY * EX;         // e_z on  TZ x (TY+4) x (TX+4)
+  static constexpr int TAB_OFF = (EZ_OFF + TZ * (TY + 4) * EX + 1) / 2 * 2;   // int4 table, 16-byte aligned
+  static constexpr int N_EYX = 4 * TY * TZ, N_EZX = 4 * TY * TZ, N_EZY = 4 * TX * TZ;
+  static constexpr int NITEMS = N_EYX + N_EZX + N_EZY;         // halo entries of e_y, e_z per field
+  static constexpr int ITEMS_PER_THREAD = (NITEMS + NT - 1) / NT;
+  static constexpr int SMEM_BYTES = (TAB_OFF + 2 * NITEMS) * 8;
+  static_assert(NS <= 8, "mbarrier area");
   static_assert(NF % NS == 0, "the ring depth must divide the number of fields");
   static_assert((PX * 8) % 16 == 0, "TMA: the innermost box extent must be a multiple of 16 bytes");
 };
 
+// The CTA's dynamic shared memory: NS ring slots of SLOT doubles, then NS mbarriers. Always indexed as an
+// array (never through a stored generic pointer), so that every access compiles to LDS with an immediate offset.
+extern __shared__ __align__(1024) double tile_smem[];
+
 // sample loader of one field for field_derivs(): shared-memory tile, compile-time strides
 template <class C>
 struct TileLoader {
-  const double* c;   // this thread's centre inside the ring slot of the field
-  __device__ __forceinline__ double operator()(int a, int k) const {
-    return c[k * (a == 0 ? 1 : (a == 1 ? C::PX : C::PX * C::PY))];
+  int c;     // index of this thread's centre inside the ring slot of the field
+  int slot;  // index of the ring slot (start of the box)
+  int ey, ez;  // this thread's entries of the e arrays
+  __device__ __forceinline__ static constexpr int stride(int a) { return a == 0 ? 1 : (a == 1 ? C::PX : C::PX * C::PY); }
+  __device__ __forceinline__ double operator()(int a, int k) const { return tile_smem[c + k * stride(a)]; }
+
+  // Mixed second derivatives (item 4): D_ab = D_a(e_b), e_b = 8 (u(+1)-u(-1)) - (u(+2)-u(-2)) along the later
+  // axis b. e_y and e_z of a point are the numerators of its own D_y, D_z; every thread publishes its pair,
+  // the entries two cells outside the tile (x halo of e_y, e_z; y halo of e_z) are computed from the box by the
+  // threads the table assigns them to, and after one barrier the outer difference reads four neighbours.
+  __device__ __forceinline__ void publish_e(double e_y, double e_z) const {
+    tile_smem[ey] = e_y;
+    tile_smem[ez] = e_z;
+    const int tid = threadIdx.x + C::TX * (threadIdx.y + C::TY * threadIdx.z);
+    const int4* tab = reinterpret_cast<const int4*>(tile_smem + C::TAB_OFF);
+#pragma unroll
+    for (int r = 0; r < C::ITEMS_PER_THREAD; ++r) {
+      const int j = tid + r * C::NT;
+      if (j < C::NITEMS) {                       // warp-uniform when NITEMS is a multiple of 32
+        const int4 t = tab[j];                   // {centre in the box, stride, destination, -}
+        const double* u = tile_smem + slot + t.x;
+        tile_smem[t.z] = d1_num(u[-2 * t.y], u[-t.y], u[t.y], u[2 * t.y]);
+      }
+    }
+    __syncthreads();
   }
-  __device__ __forceinline__ double mixed(int a, int ka, int b, int kb) const {
-    return c[ka * (a == 0 ? 1 : (a == 1 ? C::PX : C::PX * C::PY)) + kb * (b == 0 ? 1 : (b == 1 ? C::PX : C::PX * C::PY))];
-  }
+  __device__ __forceinline__ double e_y_x(int k) const { return tile_smem[ey + k]; }            // e_y at x + k
+  __device__ __forceinline__ double e_z_x(int k) const { return tile_smem[ez + k]; }            // e_z at x + k
+  __device__ __forceinline__ double e_z_y(int k) const { return tile_smem[ez + k * C::EX]; }    // e_z at y + k
 };
+
+// halo-item table of the e exchange: built once per CTA (the same for every field and tile)
+template <class C>
+__device__ __forceinline__ void build_e_table() {
+  const int tid = threadIdx.x + C::TX * (threadIdx.y + C::TY * threadIdx.z);
+  int4* tab = reinterpret_cast<int4*>(tile_smem + C::TAB_OFF);
+  for (int j = tid; j < C::NITEMS; j += C::NT) {
+    int x, y, z, st, dst;
+    if (j < C::N_EYX + C::N_EZX) {               // x halo: columns -2, -1, TX, TX+1
+      const int jj = j < C::N_EYX ? j : j - C::N_EYX;
+      const int col = jj % 4;
+      x = col < 2 ? col - 2 : C::TX + col - 2;
+      y = (jj / 4) % C::TY;
+      z = jj / (4 * C::TY);
+      if (j < C::N_EYX) { st = C::PX; dst = C::EY_OFF + (z * C::TY + y) * C::EX + (x + 2); }
+      else { st = C::PX * C::PY; dst = C::EZ_OFF + (z * (C::TY + 4) + (y + 2)) * C::EX + (x + 2); }
+    } else {                                     // y halo of e_z: rows -2, -1, TY, TY+1
+      const int jj = j - C::N_EYX - C::N_EZX;
+      x = jj % C::TX;
+      const int row = (jj / C::TX) % 4;
+      y = row < 2 ? row - 2 : C::TY + row - 2;
+      z = jj / (4 * C::TX);
+      st = C::PX * C::PY;
+      dst = C::EZ_OFF + (z * (C::TY + 4) + (y + 2)) * C::EX + (x + 2);
+    }
+    tab[j] = make_int4(((z + NG) * C::PY + (y + NG)) * C::PX + (x + C::XC), st, dst, 0);
+  }
+}
 
 struct TileCoord {   // box origin of a tile in the coordinates of its patch's tensor map, and the map
   const CUtensorMap* map;
@@ -100,20 +164,22 @@ template <class C>
 struct TileSource {
   const double* gcentre;   // global memory: field 0 at this thread's (clamped) point -- centre values
   long long fstride;
-  const double* sc;        // shared memory: this thread's centre in ring slot 0
-  double* ring;            // ring slot 0
-  uint64_t* full;          // NS mbarriers
+  int sc;                  // shared memory: index of this thread's centre in ring slot 0
+  int ey, ez;              // shared memory: this thread's entries of the e arrays
   TileCoord cur, nxt;      // this tile and the CTA's next tile
   bool has_next;
   uint32_t iter;           // tiles done by this CTA (ring phase)
 
   __device__ __forceinline__ double centre(int f) const { return __ldg(gcentre + (long long)f * fstride); }
 
+  __device__ __forceinline__ static uint64_t* full(int slot) {   // mbarrier "box landed" of a ring slot
+    return reinterpret_cast<uint64_t*>(tile_smem + C::BAR_OFF) + slot;
+  }
   template <int S>
-  __device__ __forceinline__ static void issue(double* ring, uint64_t* full, const TileCoord& t) {
+  __device__ __forceinline__ static void issue(const TileCoord& t) {
     constexpr int slot = S % C::NS, f = stream_field(S);
-    tma::mbar_expect_tx(full + slot, C::BOX_BYTES);
-    tma::load_box(ring + slot * C::SLOT, t.map, full + slot, t.x, t.y, t.z, f);
+    tma::mbar_expect_tx(full(slot), C::BOX_BYTES);
+    tma::load_box(tile_smem + slot * C::SLOT, t.map, full(slot), t.x, t.y, t.z, f);
   }
 
   template <int F>
@@ -123,11 +189,11 @@ struct TileSource {
     __syncthreads();
     if (threadIdx.x == 0 && threadIdx.y == 0 && threadIdx.z == 0) {
       constexpr int sn = s + C::NS - 1;
-      if constexpr (sn < NF) issue<sn>(ring, full, cur);
-      else if (has_next) issue<sn - NF>(ring, full, nxt);
+      if constexpr (sn < NF) issue<sn>(cur);
+      else if (has_next) issue<sn - NF>(nxt);
     }
-    tma::mbar_wait(full + s % C::NS, (iter * (NF / C::NS) + s / C::NS) & 1u);
-    return TileLoader<C>{sc + (s % C::NS) * C::SLOT};
+    tma::mbar_wait(full(s % C::NS), (iter * (NF / C::NS) + s / C::NS) & 1u);
+    return TileLoader<C>{sc + (s % C::NS) * C::SLOT, (s % C::NS) * C::SLOT, ey, ez};
   }
 };
 
