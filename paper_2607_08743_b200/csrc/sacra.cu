@@ -69,7 +69,12 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
 // Fused substage kernel: persistent CTAs, one thread per active point of a TX x TY x TZ tile; the 25 fields
 // are streamed through a TMA ring in shared memory (z4c_tile.cuh).
 // ---------------------------------------------------------------------------------------------------
-using Tile = TileCfg<16, 4, 4, 5>;
+#ifndef SACRA_TX   // tile shape (threads per CTA = TX*TY*TZ); overridable for tuning builds
+#define SACRA_TX 16
+#define SACRA_TY 4
+#define SACRA_TZ 4
+#endif
+using Tile = TileCfg<SACRA_TX, SACRA_TY, SACRA_TZ, 5>;
 
 struct alignas(64) TileMaps {   // one rank-4 (x, y, z, field) tensor map per patch of the launch
   CUtensorMap m[MAXP];
@@ -82,8 +87,21 @@ struct RkArgs {
   double* acc;
 };
 
+// Order in which z4c_point() emits the finished RHS values; the RK4 inputs of a field (u_n and, from stage 2
+// on, acc) are fetched from global memory one emit AHEAD of their use, so their latency is covered by the
+// derivative stage of a whole field.
+__host__ __device__ constexpr int emit_field(int e) {
+  constexpr int order[NF] = {19, 20, 21, 1, 2, 3, 4, 5, 6, 0, 18, 7, 17, 14, 15, 16, 22, 23, 24, 8, 9, 10, 11, 12, 13};
+  return order[e];
+}
+__host__ __device__ constexpr int next_emit(int f) {
+  for (int e = 0; e + 1 < NF; ++e)
+    if (emit_field(e) == f) return emit_field(e + 1);
+  return -1;
+}
+
 // active: out-of-range threads of a ragged tile run the same instruction stream on clamped / zero-filled data
-// (they must reach every barrier) and store nothing.
+// (they must reach every barrier) and store nothing; their prefetches read the clamped point.
 template <int EPI>
 struct Emitter {
   double* rhs;             // EPI == 0
@@ -91,24 +109,40 @@ struct Emitter {
   long long o, fstride;    // offset of field 0 at this point, field stride
   double dt;
   bool active;
-  __device__ __forceinline__ void operator()(int f, double kk) const {
-    if (!active) return;
-    const long long a = o + (long long)f * fstride;
-    if (EPI == 0) { rhs[a] = kk; return; }
-    const double un = rk.u_n[a];
+  double un_pf, acc_pf;    // prefetched u_n, acc of the field emitted next
+  template <int F>
+  __device__ __forceinline__ void prefetch() {
+    if (EPI == 0 || F < 0) return;
+    const long long a = o + (long long)F * fstride;
+    un_pf = rk.u_n[a];
+    if (EPI >= 2) acc_pf = rk.acc[a];
+  }
+  template <int F>
+  __device__ __forceinline__ void put(double kk) {
+    const long long a = o + (long long)F * fstride;
+    if (EPI == 0) {
+      if (active) rhs[a] = kk;
+      return;
+    }
+    const double un = un_pf, ac = acc_pf;
+    prefetch<next_emit(F)>();
+    double acc_new, u_new;
     if (EPI == 1) {
-      rk.acc[a] = kk;
-      rk.u_out[a] = __dadd_rn(un, __dmul_rn(dt / 2.0, kk));
+      acc_new = kk;
+      u_new = __dadd_rn(un, __dmul_rn(dt / 2.0, kk));
     } else if (EPI == 2) {
-      rk.acc[a] = __dadd_rn(rk.acc[a], __dmul_rn(2.0, kk));
-      rk.u_out[a] = __dadd_rn(un, __dmul_rn(dt / 2.0, kk));
+      acc_new = __dadd_rn(ac, __dmul_rn(2.0, kk));
+      u_new = __dadd_rn(un, __dmul_rn(dt / 2.0, kk));
     } else if (EPI == 3) {
-      rk.acc[a] = __dadd_rn(rk.acc[a], __dmul_rn(2.0, kk));
-      rk.u_out[a] = __dadd_rn(un, __dmul_rn(dt, kk));
+      acc_new = __dadd_rn(ac, __dmul_rn(2.0, kk));
+      u_new = __dadd_rn(un, __dmul_rn(dt, kk));
     } else {
-      const double S = __dmul_rn(__dadd_rn(rk.acc[a], kk), 1.0 / 6.0);
-      rk.acc[a] = S;
-      rk.u_out[a] = __dadd_rn(un, __dmul_rn(dt, S));
+      acc_new = __dmul_rn(__dadd_rn(ac, kk), 1.0 / 6.0);
+      u_new = __dadd_rn(un, __dmul_rn(dt, acc_new));
+    }
+    if (active) {
+      rk.acc[a] = acc_new;
+      rk.u_out[a] = u_new;
     }
   }
 };
@@ -186,7 +220,8 @@ __global__ void __launch_bounds__(Tile::NT, 1) k_z4c(const __grid_constant__ Pat
     for (int a = 0; a < 3; ++a) beta[a] = src.centre(F_BET + a);
     PointCoef pc;
     make_coef(p.dx, P.ko_sigma, beta, pc);
-    Emitter<EPI> emit{rhs, rk, p.offset + c, p.fstride, p.dt, active};
+    Emitter<EPI> emit{rhs, rk, p.offset + c, p.fstride, p.dt, active, 0.0, 0.0};
+    emit.template prefetch<emit_field(0)>();
     z4c_point(src, P, pc, emit);
     if (!src.has_next) break;
     t = tn;

@@ -15,7 +15,7 @@
 //
 // `Src` provides   src.field<F>()  -> sample loader of field F for field_derivs()
 //                  src.centre(F)   -> value of field F at the point
-// `Emit` provides  emit(F, k)      -> consumes the finished RHS value k of field F (KO included)
+// `Emit` provides  emit.put<F>(k)  -> consumes the finished RHS value k of field F (KO included)
 #pragma once
 #include "z4c_stencil.cuh"
 
@@ -100,7 +100,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, const
     gr[I] = sum9(gi, S.d2);                                                                        \
     if (I == 0) { dd[0] = S.d2[sym(0, 0)]; dd[1] = S.d2[sym(1, 0)]; dd[2] = S.d2[sym(2, 0)]; }     \
     else { dd[0] += S.d2[sym(0, I)]; dd[1] += S.d2[sym(1, I)]; dd[2] += S.d2[sym(2, I)]; }         \
-    emit(F_BET + I, (S.adv + P.shift_coef * src.centre(F_B + I)) + S.ko);                          \
+    emit.template put<F_BET + I>((S.adv + P.shift_coef * src.centre(F_B + I)) + S.ko);                          \
   }
   BETA_FIELD(0) BETA_FIELD(1) BETA_FIELD(2)
 #undef BETA_FIELD
@@ -136,7 +136,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, const
     lie += g[sym(I, 1)] * db[J][1] + g[sym(J, 1)] * db[I][1];                                      \
     lie += g[sym(I, 2)] * db[J][2] + g[sym(J, 2)] * db[I][2];                                      \
     const double a = -2.0 * alp * src.centre(F_A + n);                                             \
-    emit(F_G + n, (((a + S.adv) + lie) - two3 * g[n] * divb) + S.ko);                              \
+    emit.template put<F_G + n>((((a + S.adv) + lie) - two3 * g[n] * divb) + S.ko);                              \
   }
   GT_FIELD(0, 0) GT_FIELD(0, 1) GT_FIELD(0, 2) GT_FIELD(1, 1) GT_FIELD(1, 2) GT_FIELD(2, 2)
 #undef GT_FIELD
@@ -236,7 +236,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, const
 #pragma unroll
     for (int i = 0; i < 3; ++i)
       gr[i] = fma(f, fma(Auu[i][2], dW[2], fma(Auu[i][1], dW[1], Auu[i][0] * dW[0])), gr[i]);
-    emit(F_W, (S.adv + third * W * (alp * K - divb)) + S.ko);
+    emit.template put<F_W>((S.adv + third * W * (alp * K - divb)) + S.ko);
   }
   const double R = sum9(gi, Rt);                                         // R = gt^ij W^2 R_ij
 
@@ -267,7 +267,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, const
     for (int i = 0; i < 3; ++i)
       gr[i] = fma(-2.0, fma(Auu[i][2], da[2], fma(Auu[i][1], da[1], Auu[i][0] * da[0])), gr[i]);
     const double Ksrc = P.lapse_uses_khat ? Kh : K;                      // reading C
-    emit(F_ALP, (S.adv - 2.0 * alp * Ksrc) + S.ko);
+    emit.template put<F_ALP>((S.adv - 2.0 * alp * Ksrc) + S.ko);
   }
 
   // ---- K-hat and Theta: gradient term of Gt^i, and their own RHS ------------------------------------------
@@ -277,7 +277,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, const
 #pragma unroll
     for (int i = 0; i < 3; ++i) gr[i] = fma(f, row3(gi, i, S.d1), gr[i]);
     const double k = ((-lapa + alp * (AA + third * K * K)) + alp * P.kappa1 * (1.0 - P.kappa2) * Th) + S.adv;
-    emit(F_KH, k + S.ko);
+    emit.template put<F_KH>(k + S.ko);
   }
   {
     field_derivs<true, false>(src.template field<F_TH>(), pc, S);
@@ -285,16 +285,17 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, const
 #pragma unroll
     for (int i = 0; i < 3; ++i) gr[i] = fma(f, row3(gi, i, S.d1), gr[i]);
     const double k = (half * alp * ((R - AA) + two3 * K * K) - alp * P.kappa1 * (2.0 + P.kappa2) * Th) + S.adv;
-    emit(F_TH, k + S.ko);
+    emit.template put<F_TH>(k + S.ko);
   }
 
   // ---- Gt^i complete; B^i (Eq. 8; reading H: the Gt^i RHS enters without KO and without advection) --------
-#pragma unroll
-  for (int i = 0; i < 3; ++i) emit(F_GAM + i, (gr[i] + advG[i]) + koG[i]);
+  emit.template put<F_GAM + 0>((gr[0] + advG[0]) + koG[0]);
+  emit.template put<F_GAM + 1>((gr[1] + advG[1]) + koG[1]);
+  emit.template put<F_GAM + 2>((gr[2] + advG[2]) + koG[2]);
 #define B_FIELD(I)                                                                                 \
   {                                                                                                \
     field_derivs<false, false>(src.template field<F_B + I>(), pc, S);                              \
-    emit(F_B + I, ((S.adv + gr[I]) - P.eta * S.u0) + S.ko);                                        \
+    emit.template put<F_B + I>(((S.adv + gr[I]) - P.eta * S.u0) + S.ko);                                        \
   }
   B_FIELD(0) B_FIELD(1) B_FIELD(2)
 #undef B_FIELD
@@ -321,7 +322,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, const
     lie += A[sym(I, 1)] * db[J][1] + A[sym(J, 1)] * db[I][1];                                      \
     lie += A[sym(I, 2)] * db[J][2] + A[sym(J, 2)] * db[I][2];                                      \
     const double k = xtf + alp * (K * A[n] - 2.0 * aa);                                            \
-    emit(F_A + n, (((k + S.adv) + lie) - two3 * A[n] * divb) + S.ko);                              \
+    emit.template put<F_A + n>((((k + S.adv) + lie) - two3 * A[n] * divb) + S.ko);                              \
   }
     AT_FIELD(0, 0) AT_FIELD(0, 1) AT_FIELD(0, 2) AT_FIELD(1, 1) AT_FIELD(1, 2) AT_FIELD(2, 2)
 #undef AT_FIELD
