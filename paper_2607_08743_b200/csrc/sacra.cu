@@ -76,8 +76,8 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
 #endif
 using Tile = TileCfg<SACRA_TX, SACRA_TY, SACRA_TZ, 5>;
 
-struct alignas(64) TileMaps {   // one rank-4 (x, y, z, field) tensor map per patch of the launch
-  CUtensorMap m[MAXP];
+struct alignas(64) TileMaps {   // rank-4 (x, y, z, field) tensor maps of every patch of the launch (TileMapSet)
+  CUtensorMap box[MAXP], cen[MAXP], un[MAXP], acc[MAXP];
 };
 
 // EPI: 0 = store RHS; 1..4 = RK4 substage (item 11 table)
@@ -86,37 +86,21 @@ struct RkArgs {
   double* u_out;
   double* acc;
 };
+__host__ __device__ constexpr int rk_mode(int epi) { return epi == 0 ? 0 : (epi == 1 ? 1 : 2); }
 
-// Order in which z4c_point() emits the finished RHS values; the RK4 inputs of a field (u_n and, from stage 2
-// on, acc) are fetched from global memory one emit AHEAD of their use, so their latency is covered by the
-// derivative stage of a whole field.
-__host__ __device__ constexpr int emit_field(int e) {
-  constexpr int order[NF] = {19, 20, 21, 1, 2, 3, 4, 5, 6, 0, 18, 7, 17, 14, 15, 16, 22, 23, 24, 8, 9, 10, 11, 12, 13};
-  return order[e];
-}
-__host__ __device__ constexpr int next_emit(int f) {
-  for (int e = 0; e + 1 < NF; ++e)
-    if (emit_field(e) == f) return emit_field(e + 1);
-  return -1;
-}
-
-// active: out-of-range threads of a ragged tile run the same instruction stream on clamped / zero-filled data
-// (they must reach every barrier) and store nothing; their prefetches read the clamped point.
-template <int EPI>
+// Consumes the finished RHS values. The RK4 inputs never come from global loads: at stage 1 u_n is the stage
+// input itself (centre tile), from stage 2 on u_n and acc arrive through the TMA ring of TileSource.
+// active: out-of-range threads of a ragged tile run the same instruction stream on zero-filled data (they
+// must reach every barrier) and store nothing.
+template <int EPI, class Src>
 struct Emitter {
+  const Src& src;
   double* rhs;             // EPI == 0
-  RkArgs rk;
+  double* u_out;
+  double* acc;
   long long o, fstride;    // offset of field 0 at this point, field stride
   double dt;
   bool active;
-  double un_pf, acc_pf;    // prefetched u_n, acc of the field emitted next
-  template <int F>
-  __device__ __forceinline__ void prefetch() {
-    if (EPI == 0 || F < 0) return;
-    const long long a = o + (long long)F * fstride;
-    un_pf = rk.u_n[a];
-    if (EPI >= 2) acc_pf = rk.acc[a];
-  }
   template <int F>
   __device__ __forceinline__ void put(double kk) {
     const long long a = o + (long long)F * fstride;
@@ -124,8 +108,9 @@ struct Emitter {
       if (active) rhs[a] = kk;
       return;
     }
-    const double un = un_pf, ac = acc_pf;
-    prefetch<next_emit(F)>();
+    double un, ac = 0.0;
+    if (EPI == 1) un = src.centre(F);
+    else src.template rk_inputs<F>(un, ac);
     double acc_new, u_new;
     if (EPI == 1) {
       acc_new = kk;
@@ -141,8 +126,8 @@ struct Emitter {
       u_new = __dadd_rn(un, __dmul_rn(dt, acc_new));
     }
     if (active) {
-      rk.acc[a] = acc_new;
-      rk.u_out[a] = u_new;
+      acc[a] = acc_new;
+      u_out[a] = u_new;
     }
   }
 };
@@ -163,37 +148,35 @@ __device__ __forceinline__ TileId locate(const PatchBatch& B, int t) {
   id.by = b % nby; id.bz = b / nby;
   return id;
 }
+// map coordinates of the first active cell of a tile: map x coordinate c <-> storage cell c-1 (the maps start
+// one double before storage cell 0, on a 16-byte boundary), active cell i <-> storage cell i + NG
+template <class C>
+__device__ __forceinline__ TileCoord coord(const TileMaps& M, const TileId& id) {
+  return TileCoord{{&M.box[id.ip], &M.cen[id.ip], &M.un[id.ip], &M.acc[id.ip]},
+                   id.bx * C::TX + NG + 1, id.by * C::TY + NG, id.bz * C::TZ + NG};
+}
 
 template <int EPI>
 __global__ void __launch_bounds__(Tile::NT, 1) k_z4c(const __grid_constant__ PatchBatch B,
                                                      const __grid_constant__ Params P,
                                                      const __grid_constant__ TileMaps M,
-                                                     const double* __restrict__ u_in, double* __restrict__ rhs,
-                                                     const __grid_constant__ RkArgs rk) {
+                                                     double* __restrict__ rhs, const __grid_constant__ RkArgs rk) {
   using C = Tile;
+  using Src = TileSource<C, rk_mode(EPI)>;
   const int ntiles = B.first_block[B.np];
-  const bool leader = (threadIdx.x | threadIdx.y | threadIdx.z) == 0;
-
   int t = blockIdx.x;
   if (t >= ntiles) return;
   TileId id = locate<C>(B, t);
-  // tensor-map x coordinate c <-> storage cell c-1 (the map starts one double before storage cell 0, on a
-  // 16-byte boundary); the box of tile bx starts at the even coordinate bx*TX = storage cell bx*TX - 1
-  TileSource<C> src;
-  src.cur = TileCoord{&M.m[id.ip], id.bx * C::TX, id.by * C::TY, id.bz * C::TZ};
-  if (leader) {
-    for (int s = 0; s < C::NS; ++s) tma::mbar_init(TileSource<C>::full(s), 1);
+  Src src;
+  src.tid = threadIdx.x + C::TX * (threadIdx.y + C::TY * threadIdx.z);
+  src.cur = coord<C>(M, id);
+  if (src.tid == 0) {
+    for (int i = 0; i < C::NS + 2 + C::RKD; ++i) tma::mbar_init(Src::bar(i), 1);
     tma::fence_mbar_init();
   }
+  build_e_table<C>();
   __syncthreads();
-  if (leader) {   // prime the ring with the first NS-1 fields of the first tile
-    if (C::NS > 1) TileSource<C>::template issue<0>(src.cur);
-    if (C::NS > 2) TileSource<C>::template issue<1 % NF>(src.cur);
-    if (C::NS > 3) TileSource<C>::template issue<2 % NF>(src.cur);
-    if (C::NS > 4) TileSource<C>::template issue<3 % NF>(src.cur);
-    static_assert(C::NS <= 5, "prime more fields");
-  }
-  build_e_table<C>();   // visible after the first barrier of field<>()
+  if (src.tid == 0) src.prime();
   src.ey = C::EY_OFF + (threadIdx.z * C::TY + threadIdx.y) * C::EX + (threadIdx.x + 2);
   src.ez = C::EZ_OFF + (threadIdx.z * (C::TY + 4) + (threadIdx.y + 2)) * C::EX + (threadIdx.x + 2);
   src.sc = ((threadIdx.z + NG) * C::PY + (threadIdx.y + NG)) * C::PX + (threadIdx.x + C::XC);
@@ -206,23 +189,16 @@ __global__ void __launch_bounds__(Tile::NT, 1) k_z4c(const __grid_constant__ Pat
     TileId idn = id;
     if (src.has_next) {
       idn = locate<C>(B, tn);
-      src.nxt = TileCoord{&M.m[idn.ip], idn.bx * C::TX, idn.by * C::TY, idn.bz * C::TZ};
+      src.nxt = coord<C>(M, idn);
     }
     src.iter = iter;
+    src.cen = C::CEN_OFF + (iter & 1u) * NF * C::NT + src.tid;
     const int i = id.bx * C::TX + threadIdx.x, j = id.by * C::TY + threadIdx.y, k = id.bz * C::TZ + threadIdx.z;
     const bool active = (i < p.nx) & (j < p.ny) & (k < p.nz);
-    const int ic = min(i, p.nx - 1), jc = min(j, p.ny - 1), kc = min(k, p.nz - 1);
-    const long long c = (long long)(kc + NG) * p.sz + (long long)(jc + NG) * p.pitch + (ic + NG);
-    src.gcentre = u_in + p.offset + c;
-    src.fstride = p.fstride;
-    double beta[3];
-#pragma unroll
-    for (int a = 0; a < 3; ++a) beta[a] = src.centre(F_BET + a);
-    PointCoef pc;
-    make_coef(p.dx, P.ko_sigma, beta, pc);
-    Emitter<EPI> emit{rhs, rk, p.offset + c, p.fstride, p.dt, active, 0.0, 0.0};
-    emit.template prefetch<emit_field(0)>();
-    z4c_point(src, P, pc, emit);
+    const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
+    Emitter<EPI, Src> emit{src, rhs, rk.u_out, rk.acc, p.offset + c, p.fstride, p.dt, active};
+    src.begin_tile();
+    z4c_point(src, P, p.dx, emit);
     if (!src.has_next) break;
     t = tn;
     id = idn;
@@ -300,16 +276,17 @@ static EncodeTiledFn encode_tiled() {
   return fn;
 }
 
-// Rank-4 (x, y, z, field) map of one patch of state `u`. Storage cell 0 of a row sits at an odd double
-// (sacra.h: active cell 0 is 16-byte aligned and ng = 3), so the map starts ONE double earlier, which is
-// 16-byte aligned and inside the caller's buffer (patch_offset >= 1); kernel x coordinates are shifted by +1.
-static int make_map(const sacra_patch_t& a, const double* u, CUtensorMap* out) {
+// Rank-4 (x, y, z, field) map of one patch of state `u` with box bx x by x bz x bf. Storage cell 0 of a row
+// sits at an odd double (sacra.h: active cell 0 is 16-byte aligned and ng = 3), so the map starts ONE double
+// earlier, which is 16-byte aligned and inside the caller's buffer (patch_offset >= 1): map x coordinate
+// c <-> storage cell c - 1.
+static int make_map(const sacra_patch_t& a, const double* u, int bx, int by, int bz, int bf, CUtensorMap* out) {
   EncodeTiledFn enc = encode_tiled();
   if (!enc) return SACRA_ERR_CUDA;
   const cuuint64_t dims[4] = {(cuuint64_t)a.nx + 2 * NG + 1, (cuuint64_t)a.ny + 2 * NG, (cuuint64_t)a.nz + 2 * NG, NF};
   const cuuint64_t strides[3] = {(cuuint64_t)a.pitch_x * 8, (cuuint64_t)a.pitch_x * (a.ny + 2 * NG) * 8,
                                  (cuuint64_t)a.field_stride * 8};
-  const cuuint32_t box[4] = {Tile::PX, Tile::PY, Tile::PZ, 1};
+  const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, (cuuint32_t)bz, (cuuint32_t)bf};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   void* base = const_cast<double*>(u + a.patch_offset - 1);
   const CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr,
@@ -330,11 +307,11 @@ static int num_sms() {
 
 template <int EPI>
 static cudaError_t launch_one(int grid, cudaStream_t st, const PatchBatch& B, const Params& P, const TileMaps& M,
-                              const double* u_in, double* rhs, const RkArgs& rk) {
+                              double* rhs, const RkArgs& rk) {
   static const cudaError_t attr =
       cudaFuncSetAttribute(k_z4c<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile::SMEM_BYTES);
   if (attr != cudaSuccess) return attr;
-  k_z4c<EPI><<<grid, dim3(Tile::TX, Tile::TY, Tile::TZ), Tile::SMEM_BYTES, st>>>(B, P, M, u_in, rhs, rk);
+  k_z4c<EPI><<<grid, dim3(Tile::TX, Tile::TY, Tile::TZ), Tile::SMEM_BYTES, st>>>(B, P, M, rhs, rk);
   return cudaGetLastError();
 }
 
@@ -355,17 +332,22 @@ static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* 
       B.p[q] = to_dev(a);
       B.first_block[q] = nb;
       nb += ((a.nx + Tile::TX - 1) / Tile::TX) * ((a.ny + Tile::TY - 1) / Tile::TY) * ((a.nz + Tile::TZ - 1) / Tile::TZ);
-      if (int e = make_map(a, u_in, &M.m[q])) return e;
+      if (int e = make_map(a, u_in, Tile::PX, Tile::PY, Tile::PZ, 1, &M.box[q])) return e;
+      if (int e = make_map(a, u_in, Tile::TX, Tile::TY, Tile::TZ, NF, &M.cen[q])) return e;
+      if (epi >= 2) {
+        if (int e = make_map(a, u_n, Tile::TX, Tile::TY, Tile::TZ, 1, &M.un[q])) return e;
+        if (int e = make_map(a, acc, Tile::TX, Tile::TY, Tile::TZ, 1, &M.acc[q])) return e;
+      }
     }
     B.first_block[B.np] = nb;
     const int grid = nb < sms ? nb : sms;   // persistent: one CTA per SM, tiles dealt round-robin
     cudaError_t err;
     switch (epi) {
-      case 0: err = launch_one<0>(grid, st, B, P, M, u_in, rhs, rk); break;
-      case 1: err = launch_one<1>(grid, st, B, P, M, u_in, rhs, rk); break;
-      case 2: err = launch_one<2>(grid, st, B, P, M, u_in, rhs, rk); break;
-      case 3: err = launch_one<3>(grid, st, B, P, M, u_in, rhs, rk); break;
-      default: err = launch_one<4>(grid, st, B, P, M, u_in, rhs, rk); break;
+      case 0: err = launch_one<0>(grid, st, B, P, M, rhs, rk); break;
+      case 1: err = launch_one<1>(grid, st, B, P, M, rhs, rk); break;
+      case 2: err = launch_one<2>(grid, st, B, P, M, rhs, rk); break;
+      case 3: err = launch_one<3>(grid, st, B, P, M, rhs, rk); break;
+      default: err = launch_one<4>(grid, st, B, P, M, rhs, rk); break;
     }
     if (err != cudaSuccess) return SACRA_ERR_CUDA;
   }

@@ -45,9 +45,14 @@ __device__ __forceinline__ double tr_fma(const double (&a)[6], const double (&b)
 }
 
 template <class Src, class Emit>
-__device__ __forceinline__ void z4c_point(const Src& src, const Params& P, const PointCoef& pc, Emit& emit) {
+__device__ __forceinline__ void z4c_point(const Src& src, const Params& P, double h, Emit& emit) {
   const double half = 0.5, third = 1.0 / 3.0, two3 = 2.0 / 3.0;
   Stencil S;
+  PointCoef pc;
+  {
+    const double beta[3] = {src.centre(F_BET), src.centre(F_BET + 1), src.centre(F_BET + 2)};
+    make_coef(h, P.ko_sigma, beta, pc);
+  }
 
   // ---- centre values and the true inverse conformal metric (item 7; det gt is not assumed to be 1) ------
   double g[6], gi[6];

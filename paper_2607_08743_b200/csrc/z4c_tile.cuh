@@ -73,16 +73,24 @@ struct TileCfg {
   static constexpr int BOX = PX * PY * PZ;                     // doubles per box
   static constexpr int BOX_BYTES = BOX * 8;
   static constexpr int SLOT = (BOX + 15) / 16 * 16;            // doubles per ring slot (128-byte multiple)
-  // shared-memory map (in doubles): ring | mbarriers | E_y | E_z | halo-item table
-  static constexpr int BAR_OFF = NS * SLOT;                    // NS mbarriers (8 slots reserved)
+  // shared-memory map (in doubles):
+  //   ring | mbarriers | centre tiles (2 x NF x NT) | RK ring (RKD x {u_n, acc} x NT) | E_y | E_z | item table
+  static constexpr int RKD = 5;                                // depth of the RK-input ring (divides NF)
+  static constexpr int BAR_OFF = NS * SLOT;                    // NS box + 2 centre + RKD rk mbarriers (16 reserved)
+  static constexpr int CEN_OFF = BAR_OFF + 16;                 // unpadded tiles of all NF fields, double-buffered
+  static constexpr int CEN_BYTES = NF * NT * 8;
+  static constexpr int RK_OFF = CEN_OFF + 2 * NF * NT;         // slot r: u_n tile at RK_OFF + 2 r NT, acc tile + NT
   static constexpr int EX = TX + 4;                            // x extent of the e arrays (x halo of 2)
-  static constexpr int EY_OFF = BAR_OFF + 8;                   // e_y on  TZ x TY x (TX+4)
+  static constexpr int EY_OFF = RK_OFF + RKD * 2 * NT;         // e_y on  TZ x TY x (TX+4)
   static constexpr int EZ_OFF = EY_OFF + TZ * TY * EX;         // e_z on  TZ x (TY+4) x (TX+4)
-  static constexpr int TAB_OFF = (EZ_OFF + TZ * (TY + 4) * EX + 1) / 2 * 2;   // int4 table, 16-byte aligned
+  static constexpr int TAB_OFF = EZ_OFF + TZ * (TY + 4) * EX;  // int2 table
   static constexpr int N_EYX = 4 * TY * TZ, N_EZX = 4 * TY * TZ, N_EZY = 4 * TX * TZ;
   static constexpr int NITEMS = N_EYX + N_EZX + N_EZY;         // halo entries of e_y, e_z per field
   static constexpr int ITEMS_PER_THREAD = (NITEMS + NT - 1) / NT;
-  static constexpr int SMEM_BYTES = (TAB_OFF + 2 * NITEMS) * 8;
+  static constexpr int SMEM_BYTES = (TAB_OFF + NITEMS) * 8;
+  static_assert(SMEM_BYTES <= 232448, "shared memory of one CTA");
+  static_assert(NF % RKD == 0 && NS + 2 + RKD <= 16, "mbarrier area / RK ring depth");
+  static_assert((NT * 8) % 128 == 0 && SLOT % 16 == 0, "TMA destinations are 128-byte aligned");
   static_assert(NS <= 8, "mbarrier area");
   static_assert(NF % NS == 0, "the ring depth must divide the number of fields");
   static_assert((PX * 8) % 16 == 0, "TMA: the innermost box extent must be a multiple of 16 bytes");
@@ -109,14 +117,15 @@ struct TileLoader {
     tile_smem[ey] = e_y;
     tile_smem[ez] = e_z;
     const int tid = threadIdx.x + C::TX * (threadIdx.y + C::TY * threadIdx.z);
-    const int4* tab = reinterpret_cast<const int4*>(tile_smem + C::TAB_OFF);
+    const int2* tab = reinterpret_cast<const int2*>(tile_smem + C::TAB_OFF);
 #pragma unroll
     for (int r = 0; r < C::ITEMS_PER_THREAD; ++r) {
       const int j = tid + r * C::NT;
       if (j < C::NITEMS) {                       // warp-uniform when NITEMS is a multiple of 32
-        const int4 t = tab[j];                   // {centre in the box, stride, destination, -}
-        const double* u = tile_smem + slot + t.x;
-        tile_smem[t.z] = d1_num(u[-2 * t.y], u[-t.y], u[t.y], u[2 * t.y]);
+        const int2 t = tab[j];                   // {centre in the box | z-flag, destination}
+        const int st = (t.x & (1 << 30)) ? C::PX * C::PY : C::PX;
+        const double* u = tile_smem + slot + (t.x & ~(1 << 30));
+        tile_smem[t.y] = d1_num(u[-2 * st], u[-st], u[st], u[2 * st]);
       }
     }
     __syncthreads();
@@ -130,7 +139,7 @@ struct TileLoader {
 template <class C>
 __device__ __forceinline__ void build_e_table() {
   const int tid = threadIdx.x + C::TX * (threadIdx.y + C::TY * threadIdx.z);
-  int4* tab = reinterpret_cast<int4*>(tile_smem + C::TAB_OFF);
+  int2* tab = reinterpret_cast<int2*>(tile_smem + C::TAB_OFF);
   for (int j = tid; j < C::NITEMS; j += C::NT) {
     int x, y, z, st, dst;
     if (j < C::N_EYX + C::N_EZX) {               // x halo: columns -2, -1, TX, TX+1
@@ -150,50 +159,138 @@ __device__ __forceinline__ void build_e_table() {
       st = C::PX * C::PY;
       dst = C::EZ_OFF + (z * (C::TY + 4) + (y + 2)) * C::EX + (x + 2);
     }
-    tab[j] = make_int4(((z + NG) * C::PY + (y + NG)) * C::PX + (x + C::XC), st, dst, 0);
+    tab[j] = make_int2((((z + NG) * C::PY + (y + NG)) * C::PX + (x + C::XC)) | (st == C::PX ? 0 : (1 << 30)), dst);
   }
 }
 
-struct TileCoord {   // box origin of a tile in the coordinates of its patch's tensor map, and the map
-  const CUtensorMap* map;
-  int x, y, z;
+// ---- emit order = the order in which z4c_point() finishes the RHS values ------------------------------------
+// Every field is emitted right after its own derivative stage, except Gt^i, whose RHS needs the gradients of
+// K-hat and Theta and leaves after Theta.
+__host__ __device__ constexpr int emit_field(int e) {
+  constexpr int order[NF] = {19, 20, 21, 1, 2, 3, 4, 5, 6, 0, 18, 7, 17, 14, 15, 16, 22, 23, 24, 8, 9, 10, 11, 12, 13};
+  return order[e];
+}
+__host__ __device__ constexpr int emit_slot(int f) {
+  for (int e = 0; e < NF; ++e)
+    if (emit_field(e) == f) return e;
+  return -1;
+}
+// number of emits that precede the field<>() call of stream position s in program order
+__host__ __device__ constexpr int emits_before(int s) {
+  int n = 0;
+  for (int e = 0; e < NF; ++e) {
+    const int f = emit_field(e);
+    const int pos = (f >= F_GAM && f < F_GAM + 3) ? stream_slot(F_TH) : stream_slot(f);
+    if (pos < s) ++n;
+  }
+  return n;
+}
+
+struct TileMapSet {   // tensor maps of one patch (all rank 4: x, y, z, field)
+  const CUtensorMap* box;   // stage input u_in, box  PX x PY x PZ x 1   (stencil tiles)
+  const CUtensorMap* cen;   // stage input u_in, box  TX x TY x TZ x NF  (centre values of every field)
+  const CUtensorMap* un;    // u_n,              box  TX x TY x TZ x 1   (stages 2-4)
+  const CUtensorMap* acc;   // acc,              box  TX x TY x TZ x 1   (stages 2-4)
+};
+struct TileCoord {   // a tile: the maps of its patch and the map coordinates of its first active cell
+  TileMapSet m;
+  int x, y, z;       // coordinate of active cell (i0, j0, k0): storage (i0+3, j0+3, k0+3) = map (i0+4, j0+3, k0+3)
 };
 
-// Source for z4c_point(): field<F>() advances the TMA ring to field F and returns its tile loader.
-template <class C>
+// Source for z4c_point(): field<F>() advances the TMA ring to field F and returns its tile loader;
+// centre(f) reads the centre-value tile; rk_un / rk_acc read the RK-input ring (stages 2-4).
+// RK = 0: no RK inputs (plain RHS); 1: u_n is the stage input itself (centre tile); 2: u_n and acc ring.
+template <class C, int RK>
 struct TileSource {
-  const double* gcentre;   // global memory: field 0 at this thread's (clamped) point -- centre values
-  long long fstride;
+  int tid;                 // linear thread index = point of the tile
   int sc;                  // shared memory: index of this thread's centre in ring slot 0
+  int cen;                 // shared memory: this thread's entry of field 0 in the centre tile of this tile
   int ey, ez;              // shared memory: this thread's entries of the e arrays
   TileCoord cur, nxt;      // this tile and the CTA's next tile
   bool has_next;
-  uint32_t iter;           // tiles done by this CTA (ring phase)
+  uint32_t iter;           // tiles done by this CTA (ring phases)
 
-  __device__ __forceinline__ double centre(int f) const { return __ldg(gcentre + (long long)f * fstride); }
+  __device__ __forceinline__ static uint64_t* bar(int i) { return reinterpret_cast<uint64_t*>(tile_smem + C::BAR_OFF) + i; }
+  __device__ __forceinline__ static uint64_t* full(int slot) { return bar(slot); }            // box landed
+  __device__ __forceinline__ static uint64_t* cen_full(int b) { return bar(C::NS + b); }      // centre tile landed
+  __device__ __forceinline__ static uint64_t* rk_full(int r) { return bar(C::NS + 2 + r); }   // RK inputs landed
 
-  __device__ __forceinline__ static uint64_t* full(int slot) {   // mbarrier "box landed" of a ring slot
-    return reinterpret_cast<uint64_t*>(tile_smem + C::BAR_OFF) + slot;
-  }
+  __device__ __forceinline__ double centre(int f) const { return tile_smem[cen + f * C::NT]; }
+
   template <int S>
   __device__ __forceinline__ static void issue(const TileCoord& t) {
     constexpr int slot = S % C::NS, f = stream_field(S);
     tma::mbar_expect_tx(full(slot), C::BOX_BYTES);
-    tma::load_box(tile_smem + slot * C::SLOT, t.map, full(slot), t.x, t.y, t.z, f);
+    // the box starts XC cells before the first active cell in x (an even map coordinate) and NG in y, z
+    tma::load_box(tile_smem + slot * C::SLOT, t.m.box, full(slot), t.x - C::XC, t.y - NG, t.z - NG, f);
+  }
+  __device__ __forceinline__ static void issue_centre(const TileCoord& t, uint32_t buf) {
+    tma::mbar_expect_tx(cen_full(buf), C::CEN_BYTES);
+    tma::load_box(tile_smem + C::CEN_OFF + buf * NF * C::NT, t.m.cen, cen_full(buf), t.x, t.y, t.z, 0);
+  }
+  template <int E>
+  __device__ __forceinline__ static void issue_rk(const TileCoord& t) {
+    constexpr int r = E % C::RKD, f = emit_field(E);
+    tma::mbar_expect_tx(rk_full(r), 2 * C::NT * 8);
+    tma::load_box(tile_smem + C::RK_OFF + 2 * r * C::NT, t.m.un, rk_full(r), t.x, t.y, t.z, f);
+    tma::load_box(tile_smem + C::RK_OFF + (2 * r + 1) * C::NT, t.m.acc, rk_full(r), t.x, t.y, t.z, f);
+  }
+  // RK inputs of emits (LO, HI]: emit indices >= NF belong to the next tile
+  template <int LO, int HI>
+  __device__ __forceinline__ void issue_rk_range() const {
+    if constexpr (LO < HI) {
+      constexpr int e = LO + 1;
+      if constexpr (e < NF) issue_rk<e>(cur);
+      else if (has_next) issue_rk<e - NF>(nxt);
+      issue_rk_range<LO + 1, HI>();
+    }
+  }
+  // what the leader has in flight before the first field<>() call of a CTA
+  __device__ __forceinline__ void prime() const {
+    issue_centre(cur, 0);
+    issue<0>(cur);
+    if constexpr (C::NS > 2) issue<1>(cur);
+    if constexpr (C::NS > 3) issue<2>(cur);
+    if constexpr (C::NS > 4) issue<3>(cur);
+    static_assert(C::NS >= 2 && C::NS <= 5, "ring depth");
+    if constexpr (RK == 2) issue_rk_range<-1, C::RKD - 2>();
+  }
+
+  // start of a tile: every thread is done with the previous tile, whose centre buffer takes the next tile's
+  // values; then wait for this tile's centre values
+  __device__ __forceinline__ void begin_tile() const {
+    __syncthreads();
+    if (tid == 0 && has_next) issue_centre(nxt, (iter + 1) & 1u);
+    tma::mbar_wait(cen_full(iter & 1u), (iter >> 1) & 1u);
   }
 
   template <int F>
   __device__ __forceinline__ TileLoader<C> field() const {
     constexpr int s = stream_slot(F);
-    // every thread is done with the slot of field s-1: refill it with the field NS-1 ahead
+    // every thread is done with the slot of field s-1 and with every RK slot read so far: refill them
     __syncthreads();
-    if (threadIdx.x == 0 && threadIdx.y == 0 && threadIdx.z == 0) {
+    if (tid == 0) {
       constexpr int sn = s + C::NS - 1;
       if constexpr (sn < NF) issue<sn>(cur);
       else if (has_next) issue<sn - NF>(nxt);
+      if constexpr (RK == 2) {
+        // emit e may be loaded once emit e - RKD is done: through emits_before(s) + RKD - 1
+        constexpr int hi = emits_before(s) + C::RKD - 1;
+        constexpr int lo = s == 0 ? C::RKD - 2 : emits_before(s - 1) + C::RKD - 1;
+        issue_rk_range<lo, hi>();
+      }
     }
     tma::mbar_wait(full(s % C::NS), (iter * (NF / C::NS) + s / C::NS) & 1u);
     return TileLoader<C>{sc + (s % C::NS) * C::SLOT, (s % C::NS) * C::SLOT, ey, ez};
+  }
+
+  // RK inputs of field F at this point (stages 2-4): waits for the ring slot of its emit
+  template <int F>
+  __device__ __forceinline__ void rk_inputs(double& un, double& acc) const {
+    constexpr int e = emit_slot(F), r = e % C::RKD;
+    tma::mbar_wait(rk_full(r), (iter * (NF / C::RKD) + e / C::RKD) & 1u);
+    un = tile_smem[C::RK_OFF + 2 * r * C::NT + tid];
+    acc = tile_smem[C::RK_OFF + (2 * r + 1) * C::NT + tid];
   }
 };
 
