@@ -1,7 +1,7 @@
 // sacra.cu -- libsacra: C ABI (include/sacra.h) and the CUDA kernels behind it, sm_100a only.
 //
 // Kernels
-//   k_fill_ghosts   periodic halo fill, one thread per ghost-shell storage cell
+//   k_fill_ghosts   periodic halo fill, one block per storage plane and field
 //   k_z4c           derivative stage + algebra + KO + epilogue (RHS store or RK4 substage), one thread
 //                   per active point
 // There is no CPU path: every entry point enqueues kernels on the caller's stream or returns an error.
@@ -30,8 +30,8 @@ struct PatchBatch {
 };
 
 // ---------------------------------------------------------------------------------------------------
-// Periodic halo fill. The ghost shell of a patch is enumerated as storage cells of the full box; active
-// cells return immediately (they are never written, so reads and writes never overlap: item 2).
+// Periodic halo fill. Only ghost cells are written and only active cells are read (every source index is
+// wrapped into the active range), so reads and writes never overlap: item 2.
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ PatchBatch B, double* __restrict__ u) {
   int ip = 0;
@@ -39,28 +39,32 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
   while (ip + 1 < B.np && (int)blockIdx.x >= B.first_block[ip + 1]) ++ip;
   const DevPatch& p = B.p[ip];
   const int sx = p.nx + 2 * NG, sy = p.ny + 2 * NG;
-  // one block = one (row J, plane K) pair group: blockDim.x threads stride along x
-  const int row = (int)blockIdx.x - B.first_block[ip];     // 0 .. sy*sz-1
-  const int J = row % sy, Kk = row / sy;
-  const bool row_ghost = (J < NG) | (J >= NG + p.ny) | (Kk < NG) | (Kk >= NG + p.nz);
-  int j = J - NG, k = Kk - NG;
-  j = j < 0 ? j + p.ny : (j >= p.ny ? j - p.ny : j);
+  // one block = one storage plane K of one field: a ghost plane is copied whole, an active plane only
+  // has its 6 ghost rows and the 3+3 x-ghosts of its active rows
+  const int Kk = (int)blockIdx.x - B.first_block[ip];
+  int k = Kk - NG;
+  const bool plane_ghost = (k < 0) | (k >= p.nz);
   k = k < 0 ? k + p.nz : (k >= p.nz ? k - p.nz : k);
-  const long long dst_row = (long long)Kk * p.sz + (long long)J * p.pitch;
-  const long long src_row = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch;
-  for (int f = blockIdx.y; f < NF; f += gridDim.y) {
-    double* fld = u + p.offset + (long long)f * p.fstride;
-    if (row_ghost) {
-      for (int I = threadIdx.x; I < sx; I += blockDim.x) {
-        int i = I - NG;
-        i = i < 0 ? i + p.nx : (i >= p.nx ? i - p.nx : i);
-        fld[dst_row + I] = fld[src_row + i + NG];
-      }
-    } else if (threadIdx.x < 2 * NG) {
-      // active row: only the 3+3 x-ghosts
-      const int I = threadIdx.x < NG ? threadIdx.x : p.nx + threadIdx.x;   // 0..2, nx+3..nx+5
-      const int i = threadIdx.x < NG ? p.nx - NG + threadIdx.x : threadIdx.x - NG;
-      fld[dst_row + I] = fld[src_row + i + NG];
+  double* fld = u + p.offset + (long long)blockIdx.y * p.fstride;
+  double* dst = fld + (long long)Kk * p.sz;
+  const double* src = fld + (long long)(k + NG) * p.sz;
+  auto wrapx = [&](int I) { int i = I - NG; i = i < 0 ? i + p.nx : (i >= p.nx ? i - p.nx : i); return i + NG; };
+  auto wrapy = [&](int J) { int j = J - NG; j = j < 0 ? j + p.ny : (j >= p.ny ? j - p.ny : j); return j + NG; };
+  if (plane_ghost) {
+    for (int J = threadIdx.x / 32; J < sy; J += blockDim.x / 32) {     // one warp per row
+      const long long sr = (long long)wrapy(J) * p.pitch, dr = (long long)J * p.pitch;
+      for (int I = threadIdx.x % 32; I < sx; I += 32) dst[dr + I] = src[sr + wrapx(I)];
+    }
+  } else {
+    for (int r = threadIdx.x / 32; r < 2 * NG; r += blockDim.x / 32) {  // ghost rows 0..2, ny+3..ny+5
+      const int J = r < NG ? r : p.ny + r;
+      const long long sr = (long long)wrapy(J) * p.pitch, dr = (long long)J * p.pitch;
+      for (int I = threadIdx.x % 32; I < sx; I += 32) dst[dr + I] = src[sr + wrapx(I)];
+    }
+    for (int q = threadIdx.x; q < p.ny * 2 * NG; q += blockDim.x) {     // x-ghosts of the active rows
+      const int J = q / (2 * NG) + NG, c = q % (2 * NG);
+      const int I = c < NG ? c : p.nx + c;
+      dst[(long long)J * p.pitch + I] = src[(long long)J * p.pitch + wrapx(I)];
     }
   }
 }
@@ -251,10 +255,10 @@ static int launch_fill(const sacra_patch_t* p, int npatch, double* u, cudaStream
     for (int q = 0; q < B.np; ++q) {
       B.p[q] = to_dev(p[q0 + q]);
       B.first_block[q] = nb;
-      nb += (p[q0 + q].ny + 2 * NG) * (p[q0 + q].nz + 2 * NG);
+      nb += p[q0 + q].nz + 2 * NG;
     }
     B.first_block[B.np] = nb;
-    k_fill_ghosts<<<dim3(nb, NF), 64, 0, st>>>(B, u);
+    k_fill_ghosts<<<dim3(nb, NF), 256, 0, st>>>(B, u);
     if (cudaGetLastError() != cudaSuccess) return SACRA_ERR_CUDA;
   }
   return SACRA_OK;
@@ -402,6 +406,8 @@ int sacra_rk4_step(const sacra_patch_t* p, int npatch, const sacra_params_t* prm
   double* w1 = work + state_doubles;
   double* acc = work + 2 * state_doubles;
   int e;
+  // (a periodic write-through of the ghosts from the substage kernel was measured: +2.4 ms per 256^3 stage
+  //  against 0.31 ms for the fill it replaces -- DESIGN.md "What was tried")
   if ((e = launch_fill(p, npatch, u, st))) return e;
   if ((e = launch_z4c(p, npatch, prm, 1, u, nullptr, u, w0, acc, st))) return e;
   if ((e = launch_fill(p, npatch, w0, st))) return e;

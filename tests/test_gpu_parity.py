@@ -183,6 +183,24 @@ def test_substep_stage_table_against_oracle():
         acc_gpu = dev(acc_ref)
 
 
+def test_substep_leaves_ghosts_and_padding_untouched():
+    """sacra.h: u_out and acc are written on active cells only (ragged sizes incl. the minimum 6^3)"""
+    w = _smooth_random(_ragged_workload(dims=[(37, 9, 11), (6, 6, 6), (16, 33, 7)]), 31, amp=0.02)
+    ps, prm = w.patches, w.params
+    un = w.state.copy(); orc.fill_ghosts(ps, un)
+    for stage in (1, 4):
+        out = torch.full((un.size,), float("nan"), dtype=torch.float64, device="cuda")
+        acc = torch.full((un.size,), 0.5, dtype=torch.float64, device="cuda")
+        sacra.rk4_substep(ps, prm, stage, dev(un), dev(un), out, acc)
+        assert _untouched_outside_active(w, host(out))
+        acc_h, out_h = host(acc), host(out)
+        for ip in range(len(ps)):
+            for f in range(NF):
+                assert not np.any(np.isnan(w.active_view(out_h, ip, f)))
+                w.active_view(acc_h, ip, f)[...] = 0.5
+        assert np.all(acc_h == 0.5), "acc written outside the active cells (stage %d)" % stage
+
+
 def test_more_patches_than_one_launch_carries():
     dims = [(6 + (q % 3), 6, 6 + (q % 2)) for q in range(19)]
     w = _smooth_random(_ragged_workload(dims=dims), 23, amp=0.02)
