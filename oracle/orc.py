@@ -120,3 +120,11 @@ def derivs_field(p, u, f, i, j, k, sigma):
     lib().orc_derivs_field(C.byref(_patches([p])[0]), _p(u), int(f), int(i), int(j), int(k),
                            C.c_double(sigma), _p(out))
     return out[0:3], out[3:9], out[9], out[10]
+
+
+def count_ops():
+    """(adds, muls, divs) of the point-wise algebra at one point, and of the oracle's derivative bundle of one
+    field (all 3 D1, 6 D2, upwind advection, KO) -- the oracle source instantiated with a counting scalar."""
+    c = (C.c_long * 6)()
+    lib().orc_count_ops(c)
+    return tuple(c[:3]), tuple(c[3:])

@@ -29,6 +29,26 @@ template <class T> static Params<T> to_params(const orc_params& q) {
   return P;
 }
 
+// ---- operation count (for the roofline's algorithmic flops) ----------------------------
+// The same templated source instantiated with a scalar that counts its own +, -, *, / (unary minus is free).
+struct Cnt {
+  double v;
+  static long add, mul, div;
+  Cnt() : v(0) {}
+  Cnt(double x) : v(x) {}
+  Cnt(int x) : v(x) {}
+  Cnt(long x) : v((double)x) {}
+  friend Cnt operator+(Cnt a, Cnt b) { ++add; return Cnt(a.v + b.v); }
+  friend Cnt operator-(Cnt a, Cnt b) { ++add; return Cnt(a.v - b.v); }
+  friend Cnt operator*(Cnt a, Cnt b) { ++mul; return Cnt(a.v * b.v); }
+  friend Cnt operator/(Cnt a, Cnt b) { ++div; return Cnt(a.v / b.v); }
+  friend Cnt operator-(Cnt a) { return Cnt(-a.v); }
+  friend bool operator>=(Cnt a, Cnt b) { return a.v >= b.v; }
+  Cnt& operator+=(Cnt b) { ++add; v += b.v; return *this; }
+  Cnt& operator-=(Cnt b) { ++add; v -= b.v; return *this; }
+};
+long Cnt::add = 0; long Cnt::mul = 0; long Cnt::div = 0;
+
 extern "C" {
 
 int orc_num_threads(void) { return omp_get_max_threads(); }
@@ -78,6 +98,35 @@ void orc_derivs_field(const orc_patch* p_, const double* u, int field, int i, in
   for (int a = 0; a < 3; ++a) out[a] = D.d1[field][a];
   for (int a = 0; a < 6; ++a) out[3 + a] = D.d2[field][a];
   out[9] = D.adv[field]; out[10] = D.ko[field];
+}
+
+// ---- operation count: entry point (Cnt is defined above) ----------------------------------------------------
+// counts[0..2] = adds, muls, divs of the point-wise algebra (items 7-10) at one point;
+// counts[3..5] = the same for the oracle's derivative bundle of ONE field (3 D1, 6 D2, upwind, KO)
+void orc_count_ops(long* counts) {
+  Params<Cnt> P; P.kappa1 = Cnt(0.02); P.kappa2 = Cnt(0.1); P.eta = Cnt(2.0); P.shift_coef = Cnt(0.75);
+  P.ko_sigma = Cnt(0.1); P.lapse_uses_khat = 1;
+  Cnt u[NF], out[NF];
+  for (int n = 0; n < NF; ++n) u[n] = Cnt(0.01 * (n + 1));
+  u[F_W] = Cnt(0.9); u[F_ALP] = Cnt(0.8); u[F_G] = Cnt(1.1); u[F_G + 3] = Cnt(1.2); u[F_G + 5] = Cnt(0.95);
+  static Derivs<Cnt> D;
+  for (int n = 0; n < NF; ++n) {
+    for (int a = 0; a < 3; ++a) D.d1[n][a] = Cnt(0.003 * (n + a));
+    for (int a = 0; a < 6; ++a) D.d2[n][a] = Cnt(0.002 * (n - a));
+    D.adv[n] = Cnt(0.001 * n); D.ko[n] = Cnt(-0.001 * n);
+  }
+  Cnt::add = Cnt::mul = Cnt::div = 0;
+  z4c_rhs_point<Cnt>(u, D, P, out);
+  counts[0] = Cnt::add; counts[1] = Cnt::mul; counts[2] = Cnt::div;
+  // derivative bundle: a 7^3 neighbourhood of 25 fields
+  const int n = 7; const long sy = n, sz = n * n, fs = n * n * n;
+  std::vector<Cnt> buf(NF * fs);
+  for (size_t i = 0; i < buf.size(); ++i) buf[i] = Cnt(1e-3 * (double)(i % 97));
+  const Cnt* f[NF];
+  for (int q = 0; q < NF; ++q) f[q] = buf.data() + q * fs;
+  Cnt::add = Cnt::mul = Cnt::div = 0;
+  derivs_at<Cnt>(f, 3 * sz + 3 * sy + 3, sy, sz, Cnt(0.1), Cnt(0.1), D);
+  counts[3] = Cnt::add / NF; counts[4] = Cnt::mul / NF; counts[5] = Cnt::div / NF;
 }
 
 // ---- __float128 referee ------------------------------------------------------
