@@ -178,11 +178,12 @@ __global__ void __launch_bounds__(Tile::NT, 1) k_z4c(const __grid_constant__ Pat
     for (int i = 0; i < C::NS + 2 + C::RKD; ++i) tma::mbar_init(Src::bar(i), 1);
     tma::fence_mbar_init();
   }
-  build_e_table<C>();
   __syncthreads();
   if (src.tid == 0) src.prime();
   src.ey = C::EY_OFF + (threadIdx.z * C::TY + threadIdx.y) * C::EX + (threadIdx.x + 2);
   src.ez = C::EZ_OFF + (threadIdx.z * (C::TY + 4) + (threadIdx.y + 2)) * C::EX + (threadIdx.x + 2);
+  src.xh = threadIdx.x < 2 ? -2 : (threadIdx.x >= C::TX - 2 ? 2 : 0);
+  src.yh = threadIdx.y < 2 ? -2 : 2;   // rows y-2 (y = 0, 1 -> -2, -1) and y+2 (y = 2, 3 -> TY, TY+1)
   src.sc = ((threadIdx.z + NG) * C::PY + (threadIdx.y + NG)) * C::PX + (threadIdx.x + C::XC);
 
 #pragma unroll 1

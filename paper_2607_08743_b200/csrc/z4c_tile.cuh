@@ -74,7 +74,7 @@ struct TileCfg {
   static constexpr int BOX_BYTES = BOX * 8;
   static constexpr int SLOT = (BOX + 15) / 16 * 16;            // doubles per ring slot (128-byte multiple)
   // shared-memory map (in doubles):
-  //   ring | mbarriers | centre tiles (2 x NF x NT) | RK ring (RKD x {u_n, acc} x NT) | E_y | E_z | item table
+  //   ring | mbarriers | centre tiles (2 x NF x NT) | RK ring (RKD x {u_n, acc} x NT) | E_y | E_z
   static constexpr int RKD = 5;                                // depth of the RK-input ring (divides NF)
   static constexpr int BAR_OFF = NS * SLOT;                    // NS box + 2 centre + RKD rk mbarriers (16 reserved)
   static constexpr int CEN_OFF = BAR_OFF + 16;                 // unpadded tiles of all NF fields, double-buffered
@@ -83,13 +83,10 @@ struct TileCfg {
   static constexpr int EX = TX + 4;                            // x extent of the e arrays (x halo of 2)
   static constexpr int EY_OFF = RK_OFF + RKD * 2 * NT;         // e_y on  TZ x TY x (TX+4)
   static constexpr int EZ_OFF = EY_OFF + TZ * TY * EX;         // e_z on  TZ x (TY+4) x (TX+4)
-  static constexpr int TAB_OFF = EZ_OFF + TZ * (TY + 4) * EX;  // int2 table
-  static constexpr int N_EYX = 4 * TY * TZ, N_EZX = 4 * TY * TZ, N_EZY = 4 * TX * TZ;
-  static constexpr int NITEMS = N_EYX + N_EZX + N_EZY;         // halo entries of e_y, e_z per field
-  static constexpr int ITEMS_PER_THREAD = (NITEMS + NT - 1) / NT;
-  static constexpr int SMEM_BYTES = (TAB_OFF + NITEMS) * 8;
+  static constexpr int SMEM_BYTES = (EZ_OFF + TZ * (TY + 4) * EX) * 8;
   static_assert(SMEM_BYTES <= 232448, "shared memory of one CTA");
   static_assert(NF % RKD == 0 && NS + 2 + RKD <= 16, "mbarrier area / RK ring depth");
+  static_assert(TY == 4 && TX >= 4, "e exchange: one y-halo row of e_z per thread row, x-halo columns by the edge lanes");
   static_assert((NT * 8) % 128 == 0 && SLOT % 16 == 0, "TMA destinations are 128-byte aligned");
   static_assert(NS <= 8, "mbarrier area");
   static_assert(NF % NS == 0, "the ring depth must divide the number of fields");
@@ -103,30 +100,30 @@ extern __shared__ __align__(1024) double tile_smem[];
 // sample loader of one field for field_derivs(): shared-memory tile, compile-time strides
 template <class C>
 struct TileLoader {
-  int c;     // index of this thread's centre inside the ring slot of the field
-  int slot;  // index of the ring slot (start of the box)
+  int c;       // index of this thread's centre inside the ring slot of the field
   int ey, ez;  // this thread's entries of the e arrays
+  int xh;      // x-halo duty of this thread: 0 none, else the x offset (-2 or +2) of the column it also computes
+  int yh;      // y offset (-2 or +2 rows... in units of rows) of the e_z y-halo entry this thread computes
   __device__ __forceinline__ static constexpr int stride(int a) { return a == 0 ? 1 : (a == 1 ? C::PX : C::PX * C::PY); }
   __device__ __forceinline__ double operator()(int a, int k) const { return tile_smem[c + k * stride(a)]; }
+  __device__ __forceinline__ double e_at(int o, int st) const {   // inner difference along stride st at centre + o
+    const double* u = tile_smem + c + o;
+    return d1_num(u[-2 * st], u[-st], u[st], u[2 * st]);
+  }
 
   // Mixed second derivatives (item 4): D_ab = D_a(e_b), e_b = 8 (u(+1)-u(-1)) - (u(+2)-u(-2)) along the later
-  // axis b. e_y and e_z of a point are the numerators of its own D_y, D_z; every thread publishes its pair,
-  // the entries two cells outside the tile (x halo of e_y, e_z; y halo of e_z) are computed from the box by the
-  // threads the table assigns them to, and after one barrier the outer difference reads four neighbours.
+  // axis b. e_y and e_z of a point are the numerators of its own D_y, D_z; every thread publishes its pair.
+  // The entries two cells outside the tile are computed from the box without any table: thread row y computes
+  // the e_z entry of y-halo row {-2, -1, TY, TY+1}[y] in its own column (TY = 4: one each), and the lanes of
+  // columns 0, 1 / TX-2, TX-1 compute e_y, e_z two columns to their left / right. One barrier, then the outer
+  // difference reads four neighbours.
   __device__ __forceinline__ void publish_e(double e_y, double e_z) const {
     tile_smem[ey] = e_y;
     tile_smem[ez] = e_z;
-    const int tid = threadIdx.x + C::TX * (threadIdx.y + C::TY * threadIdx.z);
-    const int2* tab = reinterpret_cast<const int2*>(tile_smem + C::TAB_OFF);
-#pragma unroll
-    for (int r = 0; r < C::ITEMS_PER_THREAD; ++r) {
-      const int j = tid + r * C::NT;
-      if (j < C::NITEMS) {                       // warp-uniform when NITEMS is a multiple of 32
-        const int2 t = tab[j];                   // {centre in the box | z-flag, destination}
-        const int st = (t.x & (1 << 30)) ? C::PX * C::PY : C::PX;
-        const double* u = tile_smem + slot + (t.x & ~(1 << 30));
-        tile_smem[t.y] = d1_num(u[-2 * st], u[-st], u[st], u[2 * st]);
-      }
+    tile_smem[ez + yh * C::EX] = e_at(yh * C::PX, C::PX * C::PY);
+    if (xh) {
+      tile_smem[ey + xh] = e_at(xh, C::PX);
+      tile_smem[ez + xh] = e_at(xh, C::PX * C::PY);
     }
     __syncthreads();
   }
@@ -134,34 +131,6 @@ struct TileLoader {
   __device__ __forceinline__ double e_z_x(int k) const { return tile_smem[ez + k]; }            // e_z at x + k
   __device__ __forceinline__ double e_z_y(int k) const { return tile_smem[ez + k * C::EX]; }    // e_z at y + k
 };
-
-// halo-item table of the e exchange: built once per CTA (the same for every field and tile)
-template <class C>
-__device__ __forceinline__ void build_e_table() {
-  const int tid = threadIdx.x + C::TX * (threadIdx.y + C::TY * threadIdx.z);
-  int2* tab = reinterpret_cast<int2*>(tile_smem + C::TAB_OFF);
-  for (int j = tid; j < C::NITEMS; j += C::NT) {
-    int x, y, z, st, dst;
-    if (j < C::N_EYX + C::N_EZX) {               // x halo: columns -2, -1, TX, TX+1
-      const int jj = j < C::N_EYX ? j : j - C::N_EYX;
-      const int col = jj % 4;
-      x = col < 2 ? col - 2 : C::TX + col - 2;
-      y = (jj / 4) % C::TY;
-      z = jj / (4 * C::TY);
-      if (j < C::N_EYX) { st = C::PX; dst = C::EY_OFF + (z * C::TY + y) * C::EX + (x + 2); }
-      else { st = C::PX * C::PY; dst = C::EZ_OFF + (z * (C::TY + 4) + (y + 2)) * C::EX + (x + 2); }
-    } else {                                     // y halo of e_z: rows -2, -1, TY, TY+1
-      const int jj = j - C::N_EYX - C::N_EZX;
-      x = jj % C::TX;
-      const int row = (jj / C::TX) % 4;
-      y = row < 2 ? row - 2 : C::TY + row - 2;
-      z = jj / (4 * C::TX);
-      st = C::PX * C::PY;
-      dst = C::EZ_OFF + (z * (C::TY + 4) + (y + 2)) * C::EX + (x + 2);
-    }
-    tab[j] = make_int2((((z + NG) * C::PY + (y + NG)) * C::PX + (x + C::XC)) | (st == C::PX ? 0 : (1 << 30)), dst);
-  }
-}
 
 // ---- emit order = the order in which z4c_point() finishes the RHS values ------------------------------------
 // Every field is emitted right after its own derivative stage, except Gt^i, whose RHS needs the gradients of
@@ -206,6 +175,7 @@ struct TileSource {
   int sc;                  // shared memory: index of this thread's centre in ring slot 0
   int cen;                 // shared memory: this thread's entry of field 0 in the centre tile of this tile
   int ey, ez;              // shared memory: this thread's entries of the e arrays
+  int xh, yh;              // halo duties of the e exchange (TileLoader)
   TileCoord cur, nxt;      // this tile and the CTA's next tile
   bool has_next;
   uint32_t iter;           // tiles done by this CTA (ring phases)
@@ -281,7 +251,7 @@ struct TileSource {
       }
     }
     tma::mbar_wait(full(s % C::NS), (iter * (NF / C::NS) + s / C::NS) & 1u);
-    return TileLoader<C>{sc + (s % C::NS) * C::SLOT, (s % C::NS) * C::SLOT, ey, ez};
+    return TileLoader<C>{sc + (s % C::NS) * C::SLOT, ey, ez, xh, yh};
   }
 
   // RK inputs of field F at this point (stages 2-4): waits for the ring slot of its emit
