@@ -27,10 +27,12 @@ sys.path.insert(0, ROOT)
 METRIC = "Z4c RHS+RK4 Mpoint-updates/s FP64"
 UNIT = "Mpoint-updates/s"
 NF = 25
-# Algorithmic work per point: 16 field passes x 8 B x 25 fields per RK4 step,
-# i.e. 800 B per substage launch on average; FP64 operations per RHS evaluation + RK update (FMA = 2).
+# Algorithmic work per point: 16 field passes x 8 B x 25 fields per RK4 step, i.e. 800 B per
+# substage launch on average; FP64 work per RHS evaluation + RK update after CSE: 3 586 FP64 instructions
+# (DADD 1 803, DMUL 921, DFMA 909 per point, ncu) = 4 542 flop with FMA = 2.
 ALG_BYTES_PER_POINT_STEP = 16 * 8 * NF
-ALG_FLOP_PER_POINT_STAGE = 4560.0
+ALG_FLOP_PER_POINT_STAGE = 4542.0
+ALG_FP64_INSTR_PER_POINT_STAGE = 3586.0
 FP64_LANES_PER_SM, N_SM = 64, 148
 
 
@@ -165,12 +167,10 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    from paper_2607_08743_b200 import replicas
+
     def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replicas.max_over_ranks(x, device="cuda")
 
     w = make_workload(args.config, args.n)
     ps, prm = sacra.make_patches(w.patches), sacra.make_params(w.params)
@@ -252,7 +252,7 @@ def run_ours(args):
         return
 
     hbm_gbs, sm_max_mhz, peak_src = _peaks()
-    value = world * npts * K / (total_ms * 1e-3) / 1e6
+    value = world * npts * K / (total_ms * 1e-3) / 1e6   # every rank advances an identical patch (replicas)
     e2e_val = world * npts * K / (e2e_ms * 1e-3) / 1e6
     # roofline of the dominant kernel (the fused substage kernel), per launch, averaged over the 4 stages
     alg_bytes = ALG_BYTES_PER_POINT_STEP / 4.0 * npts
@@ -271,6 +271,10 @@ def run_ours(args):
         "kernel_ms": sub_avg, "kernel_share_of_step": 4 * sub_avg / (4 * sub_avg + 5 * fill_avg),
         "fill_ms": fill_avg, "alg_bytes_per_launch": alg_bytes, "alg_flop_per_launch": alg_flop,
         "hbm_frac": (alg_bytes / t_k / 1e9) / hbm_gbs, "alu_frac": (alg_flop / t_k / 1e12) / fp64_peak_tf,
+        # FP64 instructions against the issue rate of the FP64 pipe (64 lanes per SM and clock): the tighter ALU
+        # ceiling of this instruction mix (a quarter FMAs); measured DFMA/DADD rates: BASELINE.md section 3
+        "fp64_issue_frac": ALG_FP64_INSTR_PER_POINT_STAGE * npts / t_k /
+                           (N_SM * FP64_LANES_PER_SM * sm_max_mhz * 1e6),
         "peak_source": peak_src + "; FP64 peak = 148 SM x 64 lanes x 2 x sm_max_mhz (DESIGN.md)"})
 
     # ---- CPU oracle beside it (reported baseline, bounded sample) -----------------------------------------

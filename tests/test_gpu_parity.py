@@ -241,3 +241,49 @@ def test_pi_symmetry_with_shift_of_both_signs():
         a = w.active_view(k1, 0, f)
         assert np.max(np.abs(a - wl.PI_SIGN[f] * pi_partner(a))) == 0.0, wl.FIELD_NAMES[f]
     assert np.min(w.active_view(u, 0, wl.F_BET)) < 0 < np.max(w.active_view(u, 0, wl.F_BET))
+
+
+# ------------------------------------------------------------------------------------------- full size
+def test_full_size_config4_sampled_blocks_against_oracle():
+    """BASELINE.json configs[4] (256^3) in the launch configuration bench.py times (one sacra_rk4_step call on the
+    whole patch). The oracle cannot do 256^3 in seconds, so it recomputes SAMPLED blocks: one RK4 step has a
+    domain of dependence of 4 stages x 3 cells, so the 8^3 centre of a 32^3 periodic sub-patch cut out of the
+    same data (with wrap-around) is exact. Blocks: the two punctures, the domain corner (periodic wrap), a face,
+    and seeded random places. Increment S and new state, same tolerances as everywhere."""
+    w = wl.make(4)
+    p = w.patches[0]
+    got, S = gpu_step(w, w.state)
+    rng = np.random.default_rng(404)
+    m, core, mar = 32, 8, 12
+    c = p.nx // 2
+    centres = [(c, c, c + 20), (c, c, c - 20), (0, 0, 0), (c, 3, c), (p.nz - 2, c, 5)]
+    centres += [tuple(int(v) for v in rng.integers(0, p.nx, size=3)) for _ in range(3)]
+    # pass 1: the oracle on every block. The tolerance scales with max|S_f| over the WHOLE field, which the
+    # oracle cannot afford; the maximum over the valid interiors of all sampled blocks (the puncture blocks
+    # dominate) is a lower bound of it computed by the oracle alone, so the test is stricter than required.
+    blocks = []
+    for (kz, jy, ix) in centres:
+        ps, total = wl.make_layout([(m, m, m)], [p.dx], [p.dt], [(0.0, 0.0, 0.0)])
+        s = wl.Workload("block", ps, dict(w.params), np.zeros(total))
+        zi = (np.arange(m) + kz - m // 2) % p.nz
+        yi = (np.arange(m) + jy - m // 2) % p.ny
+        xi = (np.arange(m) + ix - m // 2) % p.nx
+        for f in range(NF):
+            s.active_view(s.state, 0, f)[...] = w.active_view(w.state, 0, f)[np.ix_(zi, yi, xi)]
+        ref = s.state.copy()
+        S_ref = orc.rk4_step(s.patches, s.params, ref)
+        blocks.append((s, ref, S_ref, zi, yi, xi))
+    sl = slice(mar, mar + core)
+    scale = [max(np.max(np.abs(b[0].active_view(b[2], 0, f)[mar:-mar, mar:-mar, mar:-mar])) for b in blocks)
+             for f in range(NF)]
+    # pass 2: element by element on the exact 8^3 cores
+    for (s, ref, S_ref, zi, yi, xi), ctr in zip(blocks, centres):
+        for f in range(NF):
+            sub = np.ix_(zi[sl], yi[sl], xi[sl])
+            a = w.active_view(S, 0, f)[sub]
+            b = s.active_view(S_ref, 0, f)[sl, sl, sl]
+            assert np.max(np.abs(a - b)) <= RTOL * (scale[f] + FLOOR), (wl.FIELD_NAMES[f], ctr)
+            un = w.active_view(got, 0, f)[sub]
+            ur = s.active_view(ref, 0, f)[sl, sl, sl]
+            assert np.all(np.abs(un - ur) <= p.dt * RTOL * (scale[f] + FLOOR) + np.spacing(np.abs(ur))), \
+                (wl.FIELD_NAMES[f], ctr)
