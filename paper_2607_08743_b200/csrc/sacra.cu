@@ -73,12 +73,15 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
 // Fused substage kernel: persistent CTAs, one thread per active point of a TX x TY x TZ tile; the 25 fields
 // are streamed through a TMA ring in shared memory (z4c_tile.cuh).
 // ---------------------------------------------------------------------------------------------------
-#ifndef SACRA_TX   // tile shape (threads per CTA = TX*TY*TZ); overridable for tuning builds
+#ifndef SACRA_TX   // tile shape (threads per CTA = TX*TY*TZ), ring depth, centre buffers, CTAs per SM: tuning builds
 #define SACRA_TX 16
 #define SACRA_TY 4
 #define SACRA_TZ 4
+#define SACRA_NS 5
+#define SACRA_CB 2
+#define SACRA_CTAS 1
 #endif
-using Tile = TileCfg<SACRA_TX, SACRA_TY, SACRA_TZ, 5>;
+using Tile = TileCfg<SACRA_TX, SACRA_TY, SACRA_TZ, SACRA_NS, SACRA_CB, SACRA_CTAS>;
 
 struct alignas(64) TileMaps {   // rank-4 (x, y, z, field) tensor maps of every patch of the launch (TileMapSet)
   CUtensorMap box[MAXP], cen[MAXP], un[MAXP], acc[MAXP];
@@ -161,7 +164,7 @@ __device__ __forceinline__ TileCoord coord(const TileMaps& M, const TileId& id) 
 }
 
 template <int EPI>
-__global__ void __launch_bounds__(Tile::NT, 1) k_z4c(const __grid_constant__ PatchBatch B,
+__global__ void __launch_bounds__(Tile::NT, Tile::CTAS) k_z4c(const __grid_constant__ PatchBatch B,
                                                      const __grid_constant__ Params P,
                                                      const __grid_constant__ TileMaps M,
                                                      double* __restrict__ rhs, const __grid_constant__ RkArgs rk) {
@@ -179,7 +182,9 @@ __global__ void __launch_bounds__(Tile::NT, 1) k_z4c(const __grid_constant__ Pat
     tma::fence_mbar_init();
   }
   __syncthreads();
-  if (src.tid == 0) src.prime();
+  src.iter = 0;
+  src.has_next = t + (int)gridDim.x < ntiles;
+  if (src.tid == 0) src.prime();   // loads of the first tile only: nxt is not needed yet
   src.ey = C::EY_OFF + (threadIdx.z * C::TY + threadIdx.y) * C::EX + (threadIdx.x + 2);
   src.ez = C::EZ_OFF + (threadIdx.z * (C::TY + 4) + (threadIdx.y + 2)) * C::EX + (threadIdx.x + 2);
   src.xh = threadIdx.x < 2 ? -2 : (threadIdx.x >= C::TX - 2 ? 2 : 0);
@@ -197,7 +202,7 @@ __global__ void __launch_bounds__(Tile::NT, 1) k_z4c(const __grid_constant__ Pat
       src.nxt = coord<C>(M, idn);
     }
     src.iter = iter;
-    src.cen = C::CEN_OFF + (iter & 1u) * NF * C::NT + src.tid;
+    src.cen = C::CEN_OFF + (C::CB == 2 ? (iter & 1u) : 0u) * NF * C::NT + src.tid;
     const int i = id.bx * C::TX + threadIdx.x, j = id.by * C::TY + threadIdx.y, k = id.bz * C::TZ + threadIdx.z;
     const bool active = (i < p.nx) & (j < p.ny) & (k < p.nz);
     const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
@@ -345,7 +350,7 @@ static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* 
       }
     }
     B.first_block[B.np] = nb;
-    const int grid = nb < sms ? nb : sms;   // persistent: one CTA per SM, tiles dealt round-robin
+    const int grid = nb < sms * Tile::CTAS ? nb : sms * Tile::CTAS;   // persistent CTAs, tiles dealt round-robin
     cudaError_t err;
     switch (epi) {
       case 0: err = launch_one<0>(grid, st, B, P, M, rhs, rk); break;

@@ -60,9 +60,11 @@ __device__ __forceinline__ void load_box(void* dst, const CUtensorMap* map, uint
 }
 }  // namespace tma
 
-template <int TX_, int TY_, int TZ_, int NS_>
+template <int TX_, int TY_, int TZ_, int NS_, int CB_, int CTAS_>
 struct TileCfg {
   static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NS = NS_;
+  static constexpr int CB = CB_;       // centre-value buffers: 2 = the next tile's values load during this tile
+  static constexpr int CTAS = CTAS_;   // CTAs per SM the launch is sized for
   static constexpr int NT = TX * TY * TZ;                      // threads = points per tile
   // box extents. x: the box must start on a 16-byte boundary of global memory (TMA rule for the innermost
   // coordinate, found by probing: an odd FP64 start coordinate raises "illegal instruction"); storage cell
@@ -74,22 +76,22 @@ struct TileCfg {
   static constexpr int BOX_BYTES = BOX * 8;
   static constexpr int SLOT = (BOX + 15) / 16 * 16;            // doubles per ring slot (128-byte multiple)
   // shared-memory map (in doubles):
-  //   ring | mbarriers | centre tiles (2 x NF x NT) | RK ring (RKD x {u_n, acc} x NT) | E_y | E_z
+  //   ring | mbarriers | centre tiles (CB x NF x NT) | RK ring (RKD x {u_n, acc} x NT) | E_y | E_z
   static constexpr int RKD = 5;                                // depth of the RK-input ring (divides NF)
   static constexpr int BAR_OFF = NS * SLOT;                    // NS box + 2 centre + RKD rk mbarriers (16 reserved)
-  static constexpr int CEN_OFF = BAR_OFF + 16;                 // unpadded tiles of all NF fields, double-buffered
+  static constexpr int CEN_OFF = BAR_OFF + 16;                 // unpadded tiles of all NF fields, CB buffers
   static constexpr int CEN_BYTES = NF * NT * 8;
-  static constexpr int RK_OFF = CEN_OFF + 2 * NF * NT;         // slot r: u_n tile at RK_OFF + 2 r NT, acc tile + NT
+  static constexpr int RK_OFF = CEN_OFF + CB * NF * NT;         // slot r: u_n tile at RK_OFF + 2 r NT, acc tile + NT
   static constexpr int EX = TX + 4;                            // x extent of the e arrays (x halo of 2)
   static constexpr int EY_OFF = RK_OFF + RKD * 2 * NT;         // e_y on  TZ x TY x (TX+4)
   static constexpr int EZ_OFF = EY_OFF + TZ * TY * EX;         // e_z on  TZ x (TY+4) x (TX+4)
   static constexpr int SMEM_BYTES = (EZ_OFF + TZ * (TY + 4) * EX) * 8;
-  static_assert(SMEM_BYTES <= 232448, "shared memory of one CTA");
+  static_assert(SMEM_BYTES * CTAS + 1024 * CTAS <= 233472, "shared memory of the CTAs of one SM");
   static_assert(NF % RKD == 0 && NS + 2 + RKD <= 16, "mbarrier area / RK ring depth");
   static_assert(TY == 4 && TX >= 4, "e exchange: one y-halo row of e_z per thread row, x-halo columns by the edge lanes");
   static_assert((NT * 8) % 128 == 0 && SLOT % 16 == 0, "TMA destinations are 128-byte aligned");
   static_assert(NS <= 8, "mbarrier area");
-  static_assert(NF % NS == 0, "the ring depth must divide the number of fields");
+  static_assert(NS >= 2 && NS <= 5, "ring depth");
   static_assert((PX * 8) % 16 == 0, "TMA: the innermost box extent must be a multiple of 16 bytes");
 };
 
@@ -187,9 +189,17 @@ struct TileSource {
 
   __device__ __forceinline__ double centre(int f) const { return tile_smem[cen + f * C::NT]; }
 
+  // ring slot and use count of stream position s of tile `it` of this CTA: global sequence number it*NF + s
+  __device__ __forceinline__ static uint32_t ring_slot(uint32_t it, int s) { return (it * NF + s) % C::NS; }
+  __device__ __forceinline__ static uint32_t ring_use(uint32_t it, int s) { return (it * NF + s) / C::NS; }
+
+  // stream position S of tile `it` (S >= NF: position S - NF of tile it + 1, if there is one)
   template <int S>
-  __device__ __forceinline__ static void issue(const TileCoord& t) {
-    constexpr int slot = S % C::NS, f = stream_field(S);
+  __device__ __forceinline__ void issue() const {
+    if (S >= NF && !has_next) return;
+    constexpr int f = stream_field(S % NF);
+    const TileCoord& t = S < NF ? cur : nxt;
+    const uint32_t slot = ring_slot(iter, S);
     tma::mbar_expect_tx(full(slot), C::BOX_BYTES);
     // the box starts XC cells before the first active cell in x (an even map coordinate) and NG in y, z
     tma::load_box(tile_smem + slot * C::SLOT, t.m.box, full(slot), t.x - C::XC, t.y - NG, t.z - NG, f);
@@ -218,20 +228,25 @@ struct TileSource {
   // what the leader has in flight before the first field<>() call of a CTA
   __device__ __forceinline__ void prime() const {
     issue_centre(cur, 0);
-    issue<0>(cur);
-    if constexpr (C::NS > 2) issue<1>(cur);
-    if constexpr (C::NS > 3) issue<2>(cur);
-    if constexpr (C::NS > 4) issue<3>(cur);
-    static_assert(C::NS >= 2 && C::NS <= 5, "ring depth");
+    issue<0>();
+    if constexpr (C::NS > 2) issue<1>();
+    if constexpr (C::NS > 3) issue<2>();
+    if constexpr (C::NS > 4) issue<3>();
     if constexpr (RK == 2) issue_rk_range<-1, C::RKD - 2>();
   }
 
-  // start of a tile: every thread is done with the previous tile, whose centre buffer takes the next tile's
-  // values; then wait for this tile's centre values
+  // start of a tile: every thread is done with the previous tile. CB = 2: its centre buffer takes the next
+  // tile's values while this tile runs. CB = 1: this tile's values can only be requested now (a second CTA on the
+  // SM covers the wait). Then wait for this tile's centre values.
   __device__ __forceinline__ void begin_tile() const {
     __syncthreads();
-    if (tid == 0 && has_next) issue_centre(nxt, (iter + 1) & 1u);
-    tma::mbar_wait(cen_full(iter & 1u), (iter >> 1) & 1u);
+    if constexpr (C::CB == 2) {
+      if (tid == 0 && has_next) issue_centre(nxt, (iter + 1) & 1u);
+      tma::mbar_wait(cen_full(iter & 1u), (iter >> 1) & 1u);
+    } else {
+      if (tid == 0 && iter > 0) issue_centre(cur, 0);
+      tma::mbar_wait(cen_full(0), iter & 1u);
+    }
   }
 
   template <int F>
@@ -240,9 +255,7 @@ struct TileSource {
     // every thread is done with the slot of field s-1 and with every RK slot read so far: refill them
     __syncthreads();
     if (tid == 0) {
-      constexpr int sn = s + C::NS - 1;
-      if constexpr (sn < NF) issue<sn>(cur);
-      else if (has_next) issue<sn - NF>(nxt);
+      issue<s + C::NS - 1>();
       if constexpr (RK == 2) {
         // emit e may be loaded once emit e - RKD is done: through emits_before(s) + RKD - 1
         constexpr int hi = emits_before(s) + C::RKD - 1;
@@ -250,8 +263,9 @@ struct TileSource {
         issue_rk_range<lo, hi>();
       }
     }
-    tma::mbar_wait(full(s % C::NS), (iter * (NF / C::NS) + s / C::NS) & 1u);
-    return TileLoader<C>{sc + (s % C::NS) * C::SLOT, ey, ez, xh, yh};
+    const uint32_t slot = ring_slot(iter, s);
+    tma::mbar_wait(full(slot), ring_use(iter, s) & 1u);
+    return TileLoader<C>{sc + (int)slot * C::SLOT, ey, ez, xh, yh};
   }
 
   // RK inputs of field F at this point (stages 2-4): waits for the ring slot of its emit
