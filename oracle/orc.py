@@ -128,3 +128,27 @@ def count_ops():
     c = (C.c_long * 6)()
     lib().orc_count_ops(c)
     return tuple(c[:3]), tuple(c[3:])
+
+
+def constraints(ps, u):
+    """H, M^x, M^y, M^z (Eqs. 20-21, vacuum) on the active cells: a state-shaped buffer, fields 0..3."""
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    con = np.zeros_like(u)
+    lib().orc_constraints(_patches(ps), len(ps), _p(u), _p(con))
+    return con
+
+
+def constraint_norms(ps, con):
+    """volume-normalised L2 norms of the four constraints over all patches (Eq. 22)"""
+    out = np.zeros(4)
+    lib().orc_constraint_norms(_patches(ps), len(ps), _p(np.ascontiguousarray(con, dtype=np.float64)), _p(out))
+    return out
+
+
+def constraints_point(u, d1, d2):
+    """constraints at one point from caller-supplied derivatives. u[25], d1[25,3], d2[25,6]."""
+    u, d1, d2 = (np.ascontiguousarray(a, dtype=np.float64) for a in (u, d1, d2))
+    assert u.shape == (NF,) and d1.shape == (NF, 3) and d2.shape == (NF, 6)
+    out = np.zeros(4)
+    lib().orc_constraints_point(_p(u), _p(d1), _p(d2), _p(out))
+    return out

@@ -240,4 +240,125 @@ inline void z4c_rhs_point(const T u[NF], const Derivs<T>& D, const Params<T>& P,
   for (int n = 0; n < NF; ++n) out[n] = rhs[n] + D.ko[n];
 }
 
+
+
+// ---------------------------------------------------------------------------------------------------
+// Constraint monitor (Eqs. 20-21), vacuum:
+//   H   = R + K^2 - K_ij K^ij                      (Eq. 20, rho_H = 0)
+//   M^i = D_j ( K^ij - gamma^ij K )                (Eq. 21, J_i = 0)
+// "R and D_j are the Ricci scalar and covariant derivative of gamma_ij": the oracle takes that
+// literally. It rebuilds the PHYSICAL metric and extrinsic curvature and their derivatives from the evolved
+// variables by the product rule (Eqs. 1-4: gamma_ij = gt_ij / W^2,
+// K_ij = (At_ij + gt_ij K / 3) / W^2, K = K-hat + 2 Theta as in item 7) and then applies the textbook
+// definitions (Christoffel symbols, Ricci tensor from their derivatives, covariant divergence). No conformal
+// identity, no assumption det gt = 1 or tr At = 0, and nothing shared with the conformal Ricci of z4c_rhs_point.
+// out[0] = H, out[1..3] = M^x, M^y, M^z.
+template <class T>
+inline void constraints_point(const T u[NF], const Derivs<T>& D, T out[4]) {
+  const T W = u[F_W], K = u[F_KH] + T(2) * u[F_TH];
+  T dW[3], ddW[3][3], dK[3];
+  for (int k = 0; k < 3; ++k) {
+    dW[k] = D.d1[F_W][k];
+    dK[k] = D.d1[F_KH][k] + T(2) * D.d1[F_TH][k];
+    for (int l = 0; l < 3; ++l) ddW[k][l] = D.d2[F_W][SYM[k][l]];
+  }
+  // physical metric gam_ij = gt_ij W^-2 and its first and second derivatives (product rule)
+  const T w2 = T(1) / (W * W);                       // W^-2
+  T dw2[3], ddw2[3][3];                              // d_k W^-2 = -2 W^-3 d_k W ; d_k d_l W^-2
+  for (int k = 0; k < 3; ++k) dw2[k] = -T(2) * w2 / W * dW[k];
+  for (int k = 0; k < 3; ++k)
+    for (int l = 0; l < 3; ++l)
+      ddw2[k][l] = T(6) * w2 / (W * W) * dW[k] * dW[l] - T(2) * w2 / W * ddW[k][l];
+  T gam[3][3], dgam[3][3][3], ddgam[3][3][3][3], Kd[3][3], dKd[3][3][3];
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) {
+      const int n = SYM[i][j];
+      const T gt = u[F_G + n];
+      const T B = u[F_A + n] + gt * K / T(3);        // W^2 K_ij
+      gam[i][j] = gt * w2;
+      Kd[i][j] = B * w2;
+      for (int k = 0; k < 3; ++k) {
+        const T dgt = D.d1[F_G + n][k];
+        dgam[k][i][j] = dgt * w2 + gt * dw2[k];
+        const T dB = D.d1[F_A + n][k] + (dgt * K + gt * dK[k]) / T(3);
+        dKd[k][i][j] = dB * w2 + B * dw2[k];
+        for (int l = 0; l < 3; ++l)
+          ddgam[k][l][i][j] = D.d2[F_G + n][SYM[k][l]] * w2 + dgt * dw2[l] + D.d1[F_G + n][l] * dw2[k] +
+                              gt * ddw2[k][l];
+      }
+    }
+  // inverse metric and its derivative: d_l gam^ij = - gam^ia gam^jb d_l gam_ab
+  const T det = gam[0][0] * (gam[1][1] * gam[2][2] - gam[1][2] * gam[1][2]) -
+                gam[0][1] * (gam[0][1] * gam[2][2] - gam[1][2] * gam[0][2]) +
+                gam[0][2] * (gam[0][1] * gam[1][2] - gam[1][1] * gam[0][2]);
+  T gi[3][3];
+  gi[0][0] = (gam[1][1] * gam[2][2] - gam[1][2] * gam[1][2]) / det;
+  gi[0][1] = (gam[0][2] * gam[1][2] - gam[0][1] * gam[2][2]) / det;
+  gi[0][2] = (gam[0][1] * gam[1][2] - gam[0][2] * gam[1][1]) / det;
+  gi[1][1] = (gam[0][0] * gam[2][2] - gam[0][2] * gam[0][2]) / det;
+  gi[1][2] = (gam[0][1] * gam[0][2] - gam[0][0] * gam[1][2]) / det;
+  gi[2][2] = (gam[0][0] * gam[1][1] - gam[0][1] * gam[0][1]) / det;
+  gi[1][0] = gi[0][1]; gi[2][0] = gi[0][2]; gi[2][1] = gi[1][2];
+  T dgi[3][3][3];
+  for (int l = 0; l < 3; ++l)
+    for (int i = 0; i < 3; ++i)
+      for (int j = 0; j < 3; ++j) {
+        T s = T(0);
+        for (int a = 0; a < 3; ++a)
+          for (int b = 0; b < 3; ++b) s += gi[i][a] * gi[j][b] * dgam[l][a][b];
+        dgi[l][i][j] = -s;
+      }
+  // Christoffel symbols of gam: first kind Gl[c][i][j], second kind G[k][i][j], and d_l G^k_ij
+  T Gl[3][3][3], dGl[3][3][3][3], G[3][3][3], dG[3][3][3][3];
+  for (int c = 0; c < 3; ++c)
+    for (int i = 0; i < 3; ++i)
+      for (int j = 0; j < 3; ++j) {
+        Gl[c][i][j] = (dgam[i][c][j] + dgam[j][c][i] - dgam[c][i][j]) / T(2);
+        for (int l = 0; l < 3; ++l)
+          dGl[l][c][i][j] = (ddgam[l][i][c][j] + ddgam[l][j][c][i] - ddgam[l][c][i][j]) / T(2);
+      }
+  for (int k = 0; k < 3; ++k)
+    for (int i = 0; i < 3; ++i)
+      for (int j = 0; j < 3; ++j) {
+        T s = T(0);
+        for (int c = 0; c < 3; ++c) s += gi[k][c] * Gl[c][i][j];
+        G[k][i][j] = s;
+        for (int l = 0; l < 3; ++l) {
+          T t = T(0);
+          for (int c = 0; c < 3; ++c) t += dgi[l][k][c] * Gl[c][i][j] + gi[k][c] * dGl[l][c][i][j];
+          dG[l][k][i][j] = t;
+        }
+      }
+  // Ricci tensor R_ij = d_k G^k_ij - d_j G^k_ik + G^k_kl G^l_ij - G^k_jl G^l_ik ; R = gam^ij R_ij
+  T R = T(0);
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) {
+      T r = T(0);
+      for (int k = 0; k < 3; ++k) {
+        r += dG[k][k][i][j] - dG[j][k][i][k];
+        for (int l = 0; l < 3; ++l) r += G[k][k][l] * G[l][i][j] - G[k][j][l] * G[l][i][k];
+      }
+      R += gi[i][j] * r;
+    }
+  // K_ij K^ij and the divergence D_j K^ij = gam^ia gam^jb (d_j K_ab - G^c_ja K_cb - G^c_jb K_ac)
+  T KK = T(0);
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j)
+      for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) KK += gi[i][a] * gi[j][b] * Kd[i][j] * Kd[a][b];
+  out[0] = R + K * K - KK;
+  for (int i = 0; i < 3; ++i) {
+    T m = T(0);
+    for (int j = 0; j < 3; ++j)
+      for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) {
+          T cov = dKd[j][a][b];
+          for (int c = 0; c < 3; ++c) cov -= G[c][j][a] * Kd[c][b] + G[c][j][b] * Kd[a][c];
+          m += gi[i][a] * gi[j][b] * cov;
+        }
+    for (int j = 0; j < 3; ++j) m -= gi[i][j] * dK[j];
+    out[1 + i] = m;
+  }
+}
+
 }  // namespace z4c_oracle

@@ -5,6 +5,7 @@
 // Plain triple loops; OpenMP over z-planes only so that the timed CPU baseline
 // uses the host cores (no blocking, no fusion, no reordering).
 #pragma once
+#include <cmath>
 #include "z4c_algebra.hpp"
 
 namespace z4c_oracle {
@@ -55,6 +56,49 @@ void rhs_patch(const Patch& p, const Params<T>& P, const T* u, T* rhs) {
         z4c_rhs_point<T>(uc, D, P, out);
         for (int n = 0; n < NF; ++n) rhs[p.offset + (long)n * p.fstride + c] = out[n];
       }
+}
+
+// f-1: constraints (H, M^x, M^y, M^z) on every active cell of a ghost-filled state; con is a state-shaped buffer
+// whose fields 0..3 receive the four constraints on active cells (everything else untouched).
+template <class T>
+void constraints_patch(const Patch& p, const T* u, T* con) {
+  const T* f[NF];
+  for (int n = 0; n < NF; ++n) f[n] = u + p.offset + (long)n * p.fstride;
+  const long sy = sy_of(p), sz = sz_of(p);
+  const T h = T(p.dx);
+#pragma omp parallel for schedule(static)
+  for (int k = 0; k < p.nz; ++k)
+    for (int j = 0; j < p.ny; ++j)
+      for (int i = 0; i < p.nx; ++i) {
+        const long c = cell(p, i + NG, j + NG, k + NG);
+        Derivs<T> D;
+        derivs_at<T>(f, c, sy, sz, h, T(0), D);
+        T uc[NF], out[4];
+        for (int n = 0; n < NF; ++n) uc[n] = f[n][c];
+        constraints_point<T>(uc, D, out);
+        for (int n = 0; n < 4; ++n) con[p.offset + (long)n * p.fstride + c] = out[n];
+      }
+}
+
+// Eq. 22: ||C||_2 = sqrt( sum_cells C^2 dV / sum_cells dV ) over all patches, plain loops
+template <class T>
+void constraint_norms(const Patch* ps, int np, const T* con, T norms[4]) {
+  T vol = T(0), acc[4] = {T(0), T(0), T(0), T(0)};
+  for (int q = 0; q < np; ++q) {
+    const Patch& p = ps[q];
+    const T dV = T(p.dx) * T(p.dx) * T(p.dx);
+    for (int k = 0; k < p.nz; ++k)
+      for (int j = 0; j < p.ny; ++j)
+        for (int i = 0; i < p.nx; ++i) {
+          const long c = cell(p, i + NG, j + NG, k + NG);
+          vol += dV;
+          for (int n = 0; n < 4; ++n) {
+            const T v = con[p.offset + (long)n * p.fstride + c];
+            acc[n] += v * v * dV;
+          }
+        }
+  }
+  for (int n = 0; n < 4; ++n) norms[n] = sqrt(acc[n] / vol);
 }
 
 // item 11, one substage. k = F(u_in) on active cells; table of item 11:

@@ -75,6 +75,21 @@ void orc_rk4_step(const orc_patch* ps, int np, const orc_params* prm, double* u,
   rk4_step<double>(v.data(), np, P, u, work, work + nstate, work + 2 * nstate, work + 3 * nstate);
 }
 
+// f-1: constraints on all active cells (con: state-shaped, fields 0..3), their norms (Eq. 22), and the point-wise
+// form with caller-supplied derivatives (analytic-derivative pins)
+void orc_constraints(const orc_patch* ps, int np, const double* u, double* con) {
+  for (int q = 0; q < np; ++q) constraints_patch<double>(to_patch(ps[q]), u, con);
+}
+void orc_constraint_norms(const orc_patch* ps, int np, const double* con, double* norms) {
+  std::vector<Patch> v; for (int q = 0; q < np; ++q) v.push_back(to_patch(ps[q]));
+  constraint_norms<double>(v.data(), np, con, norms);
+}
+void orc_constraints_point(const double* u, const double* d1, const double* d2, double* out) {
+  static thread_local Derivs<double> D;
+  std::memcpy(D.d1, d1, sizeof(D.d1)); std::memcpy(D.d2, d2, sizeof(D.d2));
+  constraints_point<double>(u, D, out);
+}
+
 // single-point algebra with caller-supplied derivatives (for analytic-derivative pins)
 // d1: [25][3], d2: [25][6] (xx xy xz yy yz zz), adv: [25], ko: [25]
 void orc_rhs_point(const orc_params* prm, const double* u, const double* d1, const double* d2,
