@@ -1,7 +1,8 @@
 /* sacra.h -- C ABI of libsacra: the B200-native (sm_100a) hot path of SACRA-K's spacetime
  * evolution (arxiv/paper_2607_08743): periodic halo fill, Z4c/BSSN right-hand side with 4th-order
  * finite differences, upwind shift advection and 6th-derivative Kreiss-Oliger dissipation, and the
- * classical RK4 update, on batches of independent uniform FP64 patches.
+ * classical RK4 update, on batches of independent uniform FP64 patches; plus the constraint monitor of the same
+ * fields (Hamiltonian and momentum constraints and their norms).
  *
  * Citations: PAPER.md:N is a line of the paper's text; "SURVEY 8(c) item k" is the written-out form of
  * the system in SURVEY.md (the paper defers the equations to Hilditch et al. 2013).
@@ -101,6 +102,23 @@ int sacra_rk4_substep(const sacra_patch_t* p, int npatch, const sacra_params_t* 
  * nine-call sequence above. */
 int sacra_rk4_step(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, double* u,
                    double* work, int64_t state_doubles, void* cuda_stream);
+
+/* Constraint monitor (Eqs. 20-21, vacuum): Hamiltonian constraint H = R + K^2 - K_ij K^ij and
+ * momentum constraint M^i = D_j (K^ij - gamma^ij K) of the physical metric gamma_ij = gt_ij / W^2 with
+ * K_ij = (At_ij + gt_ij K / 3) / W^2, K = K-hat + 2 Theta; 4th-order centred differences.
+ * u: ghosts already filled (read only). con: a state-shaped DEVICE buffer (same descriptors as u); fields 0..3 of
+ * every patch receive H, M^x, M^y, M^z on active cells; ghosts, padding and fields 4..24 are not touched.
+ * con must not alias u. */
+int sacra_constraints(const sacra_patch_t* p, int npatch, const double* u, double* con, void* cuda_stream);
+
+/* Volume-normalised L2 norms of the four constraints over the active cells of all patches (Eq. 22):
+ * norms[c] = sqrt( sum_cells C_c^2 dV / sum_cells dV ), dV = dx^3 of the cell's patch.
+ * con: output of sacra_constraints. scratch: DEVICE buffer of at least sacra_constraint_scratch_doubles(p, npatch)
+ * doubles (4 per active z-plane). norms: DEVICE double[4], written when the stream reaches the call.
+ * The reduction order is fixed: the same input gives the same bits on every run. */
+int sacra_constraint_norms(const sacra_patch_t* p, int npatch, const double* con, double* scratch, double* norms,
+                           void* cuda_stream);
+int64_t sacra_constraint_scratch_doubles(const sacra_patch_t* p, int npatch);
 
 /* Static description of a status code (never NULL). */
 const char* sacra_strerror(int code);

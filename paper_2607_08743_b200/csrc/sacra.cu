@@ -8,10 +8,12 @@
 #include <cmath>
 #include <cstdint>
 #include <cuda_runtime.h>
+#include <type_traits>
 
 #include "../../include/sacra.h"
 #include "z4c_fused.cuh"
 #include "z4c_tile.cuh"
+#include "z4c_constraints.cuh"
 
 namespace sacra {
 
@@ -163,13 +165,15 @@ __device__ __forceinline__ TileCoord coord(const TileMaps& M, const TileId& id) 
                    id.bx * C::TX + NG + 1, id.by * C::TY + NG, id.bz * C::TZ + NG};
 }
 
+// EPI 0..4: Z4c right-hand side / RK4 substage; EPI == -1: constraint monitor (rhs receives H, M^x, M^y, M^z in
+// fields 0..3)
 template <int EPI>
 __global__ void __launch_bounds__(Tile::NT, Tile::CTAS) k_z4c(const __grid_constant__ PatchBatch B,
                                                      const __grid_constant__ Params P,
                                                      const __grid_constant__ TileMaps M,
                                                      double* __restrict__ rhs, const __grid_constant__ RkArgs rk) {
   using C = Tile;
-  using Src = TileSource<C, rk_mode(EPI)>;
+  using Src = TileSource<C, rk_mode(EPI < 0 ? 0 : EPI), std::conditional_t<EPI < 0, ConStream, Z4cStream>>;
   const int ntiles = B.first_block[B.np];
   int t = blockIdx.x;
   if (t >= ntiles) return;
@@ -206,14 +210,58 @@ __global__ void __launch_bounds__(Tile::NT, Tile::CTAS) k_z4c(const __grid_const
     const int i = id.bx * C::TX + threadIdx.x, j = id.by * C::TY + threadIdx.y, k = id.bz * C::TZ + threadIdx.z;
     const bool active = (i < p.nx) & (j < p.ny) & (k < p.nz);
     const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
-    Emitter<EPI, Src> emit{src, rhs, rk.u_out, rk.acc, p.offset + c, p.fstride, p.dt, active};
+    Emitter<(EPI < 0 ? 0 : EPI), Src> emit{src, rhs, rk.u_out, rk.acc, p.offset + c, p.fstride, p.dt, active};
     src.begin_tile();
-    z4c_point(src, P, p.dx, emit);
+    if constexpr (EPI < 0) constraints_point(src, p.dx, emit);
+    else z4c_point(src, P, p.dx, emit);
     if (!src.has_next) break;
     t = tn;
     id = idn;
     src.cur = src.nxt;
   }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Norms of the constraints, Eq. 22: sqrt( sum C^2 dV / sum dV ) over the active cells of all
+// patches. Deterministic: k_con_partial sums C^2 over one storage plane per block in a fixed order (thread t sums
+// cells t, t + 256, ... of the plane; fixed-shape tree over the threads), k_con_final adds the per-plane sums in
+// plane order with one thread per constraint. The same input gives the same bits on every run.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_con_partial(const __grid_constant__ PatchBatch B, const double* __restrict__ con,
+                                                     double* __restrict__ part, int part_base) {
+  __shared__ double red[4][256];
+  int ip = 0;
+#pragma unroll 1
+  while (ip + 1 < B.np && (int)blockIdx.x >= B.first_block[ip + 1]) ++ip;
+  const DevPatch& p = B.p[ip];
+  const int k = (int)blockIdx.x - B.first_block[ip];                 // active plane
+  const double* base = con + p.offset + (long long)(k + NG) * p.sz + (long long)NG * p.pitch + NG;
+  double acc[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int q = threadIdx.x; q < p.nx * p.ny; q += 256) {
+    const long long c = (long long)(q / p.nx) * p.pitch + (q % p.nx);
+#pragma unroll
+    for (int n = 0; n < 4; ++n) {
+      const double v = base[(long long)n * p.fstride + c];
+      acc[n] = fma(v, v, acc[n]);
+    }
+  }
+#pragma unroll
+  for (int n = 0; n < 4; ++n) red[n][threadIdx.x] = acc[n];
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s)
+#pragma unroll
+      for (int n = 0; n < 4; ++n) red[n][threadIdx.x] += red[n][threadIdx.x + s];
+    __syncthreads();
+  }
+  if (threadIdx.x < 4) part[(long long)(part_base + blockIdx.x) * 4 + threadIdx.x] = red[threadIdx.x][0] * ((p.dx * p.dx) * p.dx);
+}
+// part: nplanes x 4 weighted sums, vol = sum of dV over all active cells; one block of 4 threads
+__global__ void k_con_final(const double* __restrict__ part, int nplanes, double vol, double* __restrict__ norms) {
+  const int n = threadIdx.x;
+  double s = 0.0;
+  for (int q = 0; q < nplanes; ++q) s += part[(long long)q * 4 + n];
+  norms[n] = sqrt(s / vol);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -353,6 +401,7 @@ static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* 
     const int grid = nb < sms * Tile::CTAS ? nb : sms * Tile::CTAS;   // persistent CTAs, tiles dealt round-robin
     cudaError_t err;
     switch (epi) {
+      case -1: err = launch_one<-1>(grid, st, B, P, M, rhs, rk); break;
       case 0: err = launch_one<0>(grid, st, B, P, M, rhs, rk); break;
       case 1: err = launch_one<1>(grid, st, B, P, M, rhs, rk); break;
       case 2: err = launch_one<2>(grid, st, B, P, M, rhs, rk); break;
@@ -423,6 +472,50 @@ int sacra_rk4_step(const sacra_patch_t* p, int npatch, const sacra_params_t* prm
   if ((e = launch_fill(p, npatch, w0, st))) return e;
   if ((e = launch_z4c(p, npatch, prm, 4, w0, nullptr, u, u, acc, st))) return e;
   return launch_fill(p, npatch, u, st);
+}
+
+int sacra_constraints(const sacra_patch_t* p, int npatch, const double* u, double* con, void* cuda_stream) {
+  if (!p || !u || !con) return SACRA_ERR_NULL;
+  if (int e = check_patches(p, npatch)) return e;
+  if (!aligned16(u) || !aligned16(con)) return SACRA_ERR_ALIGN;
+  if (u == con) return SACRA_ERR_BADARG;
+  const sacra_params_t none = {0.0, 0.0, 0.0, 0.0, 0.0, 1, 0};
+  return launch_z4c(p, npatch, &none, -1, u, con, nullptr, nullptr, nullptr, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int64_t sacra_constraint_scratch_doubles(const sacra_patch_t* p, int npatch) {
+  if (!p || npatch < 1) return 0;
+  int64_t planes = 0;
+  for (int q = 0; q < npatch; ++q) planes += p[q].nz > 0 ? p[q].nz : 0;
+  return 4 * planes;
+}
+
+int sacra_constraint_norms(const sacra_patch_t* p, int npatch, const double* con, double* scratch, double* norms,
+                           void* cuda_stream) {
+  if (!p || !con || !scratch || !norms) return SACRA_ERR_NULL;
+  if (int e = check_patches(p, npatch)) return e;
+  if (!aligned16(con)) return SACRA_ERR_ALIGN;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  double vol = 0.0;
+  int planes = 0;
+  for (int q0 = 0; q0 < npatch; q0 += MAXP) {
+    PatchBatch B;
+    B.np = (npatch - q0 < MAXP) ? npatch - q0 : MAXP;
+    int nb = 0;
+    for (int q = 0; q < B.np; ++q) {
+      const sacra_patch_t& a = p[q0 + q];
+      B.p[q] = to_dev(a);
+      B.first_block[q] = nb;
+      nb += a.nz;
+      vol += (double)a.nx * a.ny * a.nz * ((a.dx * a.dx) * a.dx);
+    }
+    B.first_block[B.np] = nb;
+    k_con_partial<<<nb, 256, 0, st>>>(B, con, scratch, planes);
+    if (cudaGetLastError() != cudaSuccess) return SACRA_ERR_CUDA;
+    planes += nb;
+  }
+  k_con_final<<<1, 4, 0, st>>>(scratch, planes, vol, norms);
+  return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
 }
 
 const char* sacra_strerror(int code) {

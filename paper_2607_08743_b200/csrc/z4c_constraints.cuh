@@ -1,0 +1,186 @@
+// z4c_constraints.cuh -- Hamiltonian and momentum constraints at one point.
+//
+// PAPER.md:182-192, Eqs. 20-21, vacuum:  H = R + K^2 - K_ij K^ij ,  M^i = D_j (K^ij - gamma^ij K), with R and D_j
+// those of the physical metric gamma_ij = gt_ij / W^2 and K_ij = (At_ij + gt_ij K / 3) / W^2, K = K-hat + 2 Theta
+// (Eqs. 1-4; item 7). Evaluated in the CONFORMAL variables (the oracle goes through the physical
+// metric instead), with no assumption det gt = 1 or tr At = 0:
+//   Rt    = gt^ij ( d_k Gt^k_ij - d_j Gt^k_ik + Gt^k_kl Gt^l_ij - Gt^k_jl Gt^l_ik )      Ricci scalar of gt_ij
+//   R     = W^2 Rt + 4 W Dt^i Dt_i W - 6 Dt^i W Dt_i W                                    (gamma = W^-2 gt, 3 dimensions)
+//   B_ij  = At_ij + gt_ij K / 3 = W^2 K_ij ;   K_ij K^ij = gt^ia gt^jb B_ij B_ab
+//   M^i   = W^2 { gt^ia gt^jb [ Dt_j B_ab - 2 w_j B_ab - C^c_ja B_cb - C^c_jb B_ac ] - gt^ij d_j K },
+//           w_j = d_j W / W,  C^c_ja = -( delta^c_j w_a + delta^c_a w_j - gt_ja gt^cd w_d )   (Gamma - Gt)
+// Fields are streamed one at a time like in z4c_fused.cuh (ConStream order: W, gt_ij, K-hat, Theta, At_ij); only centred
+// derivatives are needed (no advection, no KO). A diagnostic: written for clarity, every thread runs the same
+// instruction stream.
+#pragma once
+#include "z4c_stencil.cuh"
+
+namespace sacra {
+
+template <class Src, class Emit>
+__device__ __forceinline__ void constraints_point(const Src& src, double h, Emit& emit) {
+  Stencil S;
+  PointCoef pc;
+  {
+    const double zero[3] = {0.0, 0.0, 0.0};
+    make_coef(h, 0.0, zero, pc);
+  }
+  // ---- derivatives, field by field ---------------------------------------------------------------------------
+  double dW[3], ddW[6];
+  field_derivs<true, true, false>(src.template field<F_W>(), pc, S);
+  const double W = S.u0;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) dW[k] = S.d1[k];
+#pragma unroll
+  for (int n = 0; n < 6; ++n) ddW[n] = S.d2[n];
+
+  double g[6], dg[3][6], ddg[6][6];   // ddg[lm][ij] = d_l d_m gt_ij
+#define GT_FIELD(N)                                                                  \
+  {                                                                                  \
+    field_derivs<true, true, false>(src.template field<F_G + N>(), pc, S);           \
+    g[N] = S.u0;                                                                     \
+    _Pragma("unroll") for (int k = 0; k < 3; ++k) dg[k][N] = S.d1[k];                \
+    _Pragma("unroll") for (int m = 0; m < 6; ++m) ddg[m][N] = S.d2[m];               \
+  }
+  GT_FIELD(0) GT_FIELD(1) GT_FIELD(2) GT_FIELD(3) GT_FIELD(4) GT_FIELD(5)
+#undef GT_FIELD
+
+  double K, dK[3];
+  field_derivs<true, false, false>(src.template field<F_KH>(), pc, S);
+  K = S.u0;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) dK[k] = S.d1[k];
+  field_derivs<true, false, false>(src.template field<F_TH>(), pc, S);
+  K += 2.0 * S.u0;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) dK[k] += 2.0 * S.d1[k];
+
+  double B[6], dB[3][6];              // B_ij = At_ij + gt_ij K / 3 and its gradient
+#define AT_FIELD(N)                                                                  \
+  {                                                                                  \
+    field_derivs<true, false, false>(src.template field<F_A + N>(), pc, S);          \
+    B[N] = S.u0 + g[N] * K / 3.0;                                                    \
+    _Pragma("unroll") for (int k = 0; k < 3; ++k)                                    \
+      dB[k][N] = S.d1[k] + (dg[k][N] * K + g[N] * dK[k]) / 3.0;                      \
+  }
+  AT_FIELD(0) AT_FIELD(1) AT_FIELD(2) AT_FIELD(3) AT_FIELD(4) AT_FIELD(5)
+#undef AT_FIELD
+
+  // ---- inverse conformal metric and its gradient -----------------------------------------------------------------
+  double gi[6];
+  {
+    const double gxx = g[0], gxy = g[1], gxz = g[2], gyy = g[3], gyz = g[4], gzz = g[5];
+    const double det = (gxx * (gyy * gzz - gyz * gyz) - gxy * (gxy * gzz - gyz * gxz)) + gxz * (gxy * gyz - gyy * gxz);
+    gi[0] = (gyy * gzz - gyz * gyz) / det;
+    gi[1] = (gxz * gyz - gxy * gzz) / det;
+    gi[2] = (gxy * gyz - gxz * gyy) / det;
+    gi[3] = (gxx * gzz - gxz * gxz) / det;
+    gi[4] = (gxy * gxz - gxx * gyz) / det;
+    gi[5] = (gxx * gyy - gxy * gxy) / det;
+  }
+  double dgi[3][6];                   // d_l gt^ij = - gt^ia gt^jb d_l gt_ab
+#pragma unroll
+  for (int l = 0; l < 3; ++l)
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int j = i; j < 3; ++j) {
+        double s = 0.0;
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+          for (int b = 0; b < 3; ++b) s += gi[sym(i, a)] * gi[sym(j, b)] * dg[l][sym(a, b)];
+        dgi[l][sym(i, j)] = -s;
+      }
+  // ---- Christoffel symbols of gt: Gl[c][ij] first kind, Gu[k][ij] second kind -----------------------------------
+  double Gl[3][6], Gu[3][6];
+#pragma unroll
+  for (int c = 0; c < 3; ++c)
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int j = i; j < 3; ++j) Gl[c][sym(i, j)] = 0.5 * ((dg[i][sym(c, j)] + dg[j][sym(c, i)]) - dg[c][sym(i, j)]);
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+#pragma unroll
+    for (int n = 0; n < 6; ++n) Gu[k][n] = (gi[sym(k, 0)] * Gl[0][n] + gi[sym(k, 1)] * Gl[1][n]) + gi[sym(k, 2)] * Gl[2][n];
+
+  // ---- Ricci scalar of gt from the derivatives of its Christoffel symbols --------------------------------------
+  double Rt = 0.0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      double r = 0.0;
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        // d_k Gt^k_ij = d_k gt^kl Gt_lij + gt^kl d_k Gt_lij ,  d_k Gt_lij = (d_k d_i gt_lj + d_k d_j gt_li - d_k d_l gt_ij)/2
+        // d_j Gt^k_ik = d_j gt^kl Gt_lik + gt^kl d_j Gt_lik
+#pragma unroll
+        for (int l = 0; l < 3; ++l) {
+          const double dGl_k = 0.5 * ((ddg[sym(k, i)][sym(l, j)] + ddg[sym(k, j)][sym(l, i)]) - ddg[sym(k, l)][sym(i, j)]);
+          const double dGl_j = 0.5 * ((ddg[sym(j, i)][sym(l, k)] + ddg[sym(j, k)][sym(l, i)]) - ddg[sym(j, l)][sym(i, k)]);
+          r += (dgi[k][sym(k, l)] * Gl[l][sym(i, j)] + gi[sym(k, l)] * dGl_k) -
+               (dgi[j][sym(k, l)] * Gl[l][sym(i, k)] + gi[sym(k, l)] * dGl_j);
+          r += Gu[k][sym(k, l)] * Gu[l][sym(i, j)] - Gu[k][sym(j, l)] * Gu[l][sym(i, k)];
+        }
+      }
+      Rt += gi[sym(i, j)] * r;
+    }
+  // ---- conformal factor: R = W^2 Rt + 4 W Dt^2 W - 6 |Dt W|^2 -----------------------------------------------------
+  double lapW = 0.0, dWdW = 0.0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      const int n = sym(i, j);
+      lapW += gi[n] * (((ddW[n] - Gu[0][n] * dW[0]) - Gu[1][n] * dW[1]) - Gu[2][n] * dW[2]);
+      dWdW += gi[n] * dW[i] * dW[j];
+    }
+  const double R = W * W * Rt + 4.0 * W * lapW - 6.0 * dWdW;
+  // ---- K_ij K^ij = gt^ia gt^jb B_ij B_ab -----------------------------------------------------------------------------
+  double Bu[3][3];                    // B^i_b = gt^ia B_ab
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int b = 0; b < 3; ++b)
+      Bu[i][b] = (gi[sym(i, 0)] * B[sym(0, b)] + gi[sym(i, 1)] * B[sym(1, b)]) + gi[sym(i, 2)] * B[sym(2, b)];
+  double BB = 0.0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) BB += Bu[i][j] * Bu[j][i];
+  emit.template put<0>(R + K * K - BB);
+
+  // ---- momentum constraint ------------------------------------------------------------------------------------------
+  double w[3], wu[3];                 // w_j = d_j W / W, w^c = gt^cd w_d
+#pragma unroll
+  for (int j = 0; j < 3; ++j) w[j] = dW[j] / W;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) wu[c] = (gi[sym(c, 0)] * w[0] + gi[sym(c, 1)] * w[1]) + gi[sym(c, 2)] * w[2];
+  double M[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+  for (int j = 0; j < 3; ++j)
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+      for (int b = 0; b < 3; ++b) {
+        double cov = dB[j][sym(a, b)] - 2.0 * w[j] * B[sym(a, b)];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          // Gamma^c_ja = Gt^c_ja + C^c_ja ,  C^c_ja = -( delta^c_j w_a + delta^c_a w_j - gt_ja w^c )
+          const double Cja = -(((c == j) ? w[a] : 0.0) + ((c == a) ? w[j] : 0.0) - g[sym(j, a)] * wu[c]);
+          const double Cjb = -(((c == j) ? w[b] : 0.0) + ((c == b) ? w[j] : 0.0) - g[sym(j, b)] * wu[c]);
+          cov -= (Gu[c][sym(j, a)] + Cja) * B[sym(c, b)] + (Gu[c][sym(j, b)] + Cjb) * B[sym(a, c)];
+        }
+#pragma unroll
+        for (int i = 0; i < 3; ++i) M[i] += gi[sym(i, a)] * gi[sym(j, b)] * cov;
+      }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) M[i] -= (gi[sym(i, 0)] * dK[0] + gi[sym(i, 1)] * dK[1]) + gi[sym(i, 2)] * dK[2];
+  emit.template put<1>(W * W * M[0]);
+  emit.template put<2>(W * W * M[1]);
+  emit.template put<3>(W * W * M[2]);
+}
+
+}  // namespace sacra

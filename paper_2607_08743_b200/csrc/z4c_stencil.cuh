@@ -70,7 +70,8 @@ __device__ __forceinline__ double d1_num(double um2, double um1, double up1, dou
 // exactly, s_k -> s_k, beta -> -beta. a_k is one subtraction of two samples, so its round-off scales with the
 // field's variation like every other difference here. The oracle evaluates item 5 as written; the two agree
 // to a few ulp of the advection term.
-template <bool D1, bool D2, class Ld>
+// AK = false leaves the advection and KO terms out (the constraint monitor needs only the centred derivatives).
+template <bool D1, bool D2, bool AK = true, class Ld>
 __device__ __forceinline__ void field_derivs(const Ld& ld, const PointCoef& c, Stencil& S) {
   static_assert(D1 || !D2, "the mixed second derivatives reuse the numerators of D_y, D_z");
   const double u0 = ld(0, 0);
@@ -78,9 +79,18 @@ __device__ __forceinline__ void field_derivs(const Ld& ld, const PointCoef& c, S
   double adv = 0.0, q = 0.0, num[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
-    const double m3 = ld(a, -3), m2 = ld(a, -2), m1 = ld(a, -1);
-    const double p1 = ld(a, 1), p2 = ld(a, 2), p3 = ld(a, 3);
-    const double a1 = p1 - m1, a2 = p2 - m2, a3 = p3 - m3;            // antisymmetric differences
+    const double m2 = ld(a, -2), m1 = ld(a, -1), p1 = ld(a, 1), p2 = ld(a, 2);
+    const double a1 = p1 - m1, a2 = p2 - m2;                          // antisymmetric differences
+    if (!AK) {
+      if (D1) {
+        num[a] = fma(8.0, a1, -a2);
+        S.d1[a] = num[a] * c.inv12h;
+      }
+      if (D2) S.d2[sym(a, a)] = fma(16.0, (p1 - u0) + (m1 - u0), -((p2 - u0) + (m2 - u0))) * c.inv12h2;
+      continue;
+    }
+    const double m3 = ld(a, -3), p3 = ld(a, 3);
+    const double a3 = p3 - m3;
     if (D1) {
       num[a] = fma(8.0, a1, -a2);                                     // item 3 (8 a1 is exact)
       S.d1[a] = num[a] * c.inv12h;

@@ -29,6 +29,26 @@ __host__ __device__ constexpr int stream_slot(int f) {
   return -1;
 }
 
+// the fields a kernel streams, in order: the full Z4c right-hand side, and the constraint monitor (SURVEY 8(f) f-1:
+// W, gt_ij, K-hat, Theta, At_ij -- the gauge fields and Gt^i do not enter Eqs. 20-21)
+struct Z4cStream {
+  static constexpr int N = NF;
+  __host__ __device__ static constexpr int field(int s) { return stream_field(s); }
+  __host__ __device__ static constexpr int slot(int f) { return stream_slot(f); }
+};
+struct ConStream {
+  static constexpr int N = 15;
+  __host__ __device__ static constexpr int field(int s) {
+    constexpr int order[N] = {0, 1, 2, 3, 4, 5, 6, 7, 17, 8, 9, 10, 11, 12, 13};
+    return order[s];
+  }
+  __host__ __device__ static constexpr int slot(int f) {
+    for (int s = 0; s < N; ++s)
+      if (field(s) == f) return s;
+    return -1;
+  }
+};
+
 namespace tma {
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
@@ -171,7 +191,7 @@ struct TileCoord {   // a tile: the maps of its patch and the map coordinates of
 // Source for z4c_point(): field<F>() advances the TMA ring to field F and returns its tile loader;
 // centre(f) reads the centre-value tile; rk_un / rk_acc read the RK-input ring (stages 2-4).
 // RK = 0: no RK inputs (plain RHS); 1: u_n is the stage input itself (centre tile); 2: u_n and acc ring.
-template <class C, int RK>
+template <class C, int RK, class Stream = Z4cStream>
 struct TileSource {
   int tid;                 // linear thread index = point of the tile
   int sc;                  // shared memory: index of this thread's centre in ring slot 0
@@ -190,15 +210,15 @@ struct TileSource {
   __device__ __forceinline__ double centre(int f) const { return tile_smem[cen + f * C::NT]; }
 
   // ring slot and use count of stream position s of tile `it` of this CTA: global sequence number it*NF + s
-  __device__ __forceinline__ static uint32_t ring_slot(uint32_t it, int s) { return (it * NF + s) % C::NS; }
-  __device__ __forceinline__ static uint32_t ring_use(uint32_t it, int s) { return (it * NF + s) / C::NS; }
+  __device__ __forceinline__ static uint32_t ring_slot(uint32_t it, int s) { return (it * Stream::N + s) % C::NS; }
+  __device__ __forceinline__ static uint32_t ring_use(uint32_t it, int s) { return (it * Stream::N + s) / C::NS; }
 
   // stream position S of tile `it` (S >= NF: position S - NF of tile it + 1, if there is one)
   template <int S>
   __device__ __forceinline__ void issue() const {
-    if (S >= NF && !has_next) return;
-    constexpr int f = stream_field(S % NF);
-    const TileCoord& t = S < NF ? cur : nxt;
+    if (S >= Stream::N && !has_next) return;
+    constexpr int f = Stream::field(S % Stream::N);
+    const TileCoord& t = S < Stream::N ? cur : nxt;
     const uint32_t slot = ring_slot(iter, S);
     tma::mbar_expect_tx(full(slot), C::BOX_BYTES);
     // the box starts XC cells before the first active cell in x (an even map coordinate) and NG in y, z
@@ -251,7 +271,8 @@ struct TileSource {
 
   template <int F>
   __device__ __forceinline__ TileLoader<C> field() const {
-    constexpr int s = stream_slot(F);
+    constexpr int s = Stream::slot(F);
+    static_assert(s >= 0, "field not in this kernel's stream");
     // every thread is done with the slot of field s-1 and with every RK slot read so far: refill them
     __syncthreads();
     if (tid == 0) {

@@ -18,7 +18,8 @@ NF = 25
 NG = 3
 OK, ERR_NULL, ERR_BADARG, ERR_UNSUPPORTED, ERR_ALIGN, ERR_CUDA = 0, -1, -2, -3, -4, -5
 EXPORTS = ("sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4_step",
-           "sacra_strerror", "sacra_version")
+           "sacra_strerror", "sacra_version",
+           "sacra_constraints", "sacra_constraint_norms", "sacra_constraint_scratch_doubles")
 
 
 class SacraPatch(C.Structure):
@@ -50,7 +51,11 @@ def _load():
     lib.sacra_z4c_rhs.argtypes = [vp, i32, vp, dp, dp, vp]
     lib.sacra_rk4_substep.argtypes = [vp, i32, vp, i32, dp, dp, dp, dp, vp]
     lib.sacra_rk4_step.argtypes = [vp, i32, vp, dp, dp, i64, vp]
-    for n in EXPORTS[:4]:
+    lib.sacra_constraints.argtypes = [vp, i32, dp, dp, vp]
+    lib.sacra_constraint_norms.argtypes = [vp, i32, dp, dp, dp, vp]
+    lib.sacra_constraint_scratch_doubles.argtypes = [vp, i32]
+    lib.sacra_constraint_scratch_doubles.restype = C.c_int64
+    for n in EXPORTS[:4] + EXPORTS[6:8]:
         getattr(lib, n).restype = C.c_int
     lib.sacra_strerror.argtypes = [C.c_int]
     lib.sacra_strerror.restype = C.c_char_p
@@ -142,3 +147,21 @@ def rk4_step(patches, params, u, work, state_doubles=None, stream=None):
         state_doubles = u.numel()
     _check(lib.sacra_rk4_step(ps, len(ps) if ps is not None else 0, _ref(pr), _ptr(u), _ptr(work),
                               int(state_doubles), _stream(stream)))
+
+
+def constraints(patches, u, con, stream=None):
+    """H, M^x, M^y, M^z into fields 0..3 of the state-shaped buffer con (Eqs. 20-21)."""
+    ps = make_patches(patches) if patches is not None else None
+    _check(lib.sacra_constraints(ps, len(ps) if ps is not None else 0, _ptr(u), _ptr(con), _stream(stream)))
+
+
+def constraint_scratch_doubles(patches) -> int:
+    ps = make_patches(patches)
+    return int(lib.sacra_constraint_scratch_doubles(ps, len(ps)))
+
+
+def constraint_norms(patches, con, scratch, norms, stream=None):
+    """norms: CUDA float64 tensor of 4 (Eq. 22); scratch: >= constraint_scratch_doubles(patches)."""
+    ps = make_patches(patches) if patches is not None else None
+    _check(lib.sacra_constraint_norms(ps, len(ps) if ps is not None else 0, _ptr(con), _ptr(scratch), _ptr(norms),
+                                      _stream(stream)))
