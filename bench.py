@@ -232,6 +232,25 @@ def run_ours(args):
     sub_avg = sum(sub_ms) / len(sub_ms)
     fill_avg = sum(fill_ms) / len(fill_ms)
 
+    # ---- constraint monitor on the evolved state: Eqs. 20-22, timed beside the step ------------
+    con = work[:n]
+    scratch = torch.zeros(sacra.constraint_scratch_doubles(ps), dtype=torch.float64, device="cuda")
+    norms = torch.zeros(4, dtype=torch.float64, device="cuda")
+    mon_ms = []
+    for it in range(W + K):
+        e = [ev(), ev(), ev()]
+        e[0].record(stream)
+        sacra.constraints(ps, u, con)
+        e[1].record(stream)
+        sacra.constraint_norms(ps, con, scratch, norms)
+        e[2].record(stream)
+        torch.cuda.synchronize()
+        if it >= W:
+            mon_ms.append((e[0].elapsed_time(e[1]), e[1].elapsed_time(e[2])))
+    con_ms = sum(m[0] for m in mon_ms) / len(mon_ms)
+    nrm_ms = sum(m[1] for m in mon_ms) / len(mon_ms)
+    norms_host = [float(v) for v in norms.cpu()]
+
     # ---- end to end with HOST buffers: H2D of the state, one step, D2H of the new state, every step ----
     barrier()
     e0, e1 = ev(), ev()
@@ -280,11 +299,13 @@ def run_ours(args):
     # ---- CPU oracle beside it (reported baseline, bounded sample) -----------------------------------------
     cpu = None
     if not args.no_cpu:
-        s = oracle_sample(w, args.oracle_n or 96)
-        ts, cores = time_oracle(s, 1, 1 if s.npoints <= 64 ** 3 else 0)
-        cpu = {"value": s.npoints / ts[0] / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": "central %d^3 block of %s as a periodic patch, 1 RK4 step (%.1f s)"
-                         % (s.patches[0].nx, w.name, ts[0])}
+        # bounded sample: about 10-20 s of oracle time on the box's host cores
+        s = oracle_sample(w, args.oracle_n or 160)
+        nst = 4 if s.npoints > 128 ** 3 else 8
+        ts, cores = time_oracle(s, nst, 0)
+        cpu = {"value": s.npoints * len(ts) / sum(ts) / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "central %d^3 block of %s as a periodic patch, %d RK4 steps (%.1f s)"
+                         % (s.patches[0].nx, w.name, len(ts), sum(ts))}
 
     state_bytes = n * 8
     out = {
@@ -298,6 +319,10 @@ def run_ours(args):
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes,
                 "ms_per_step": e2e_ms / K},
         "gpu_launches": 9 * K, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
+        # the constraint monitor on the state after the timed steps: 15 fields read + 4 written = 152 B per point
+        "constraint_monitor": {"constraints_ms": con_ms, "norms_ms": nrm_ms, "Mpoints_per_s": npts / (con_ms * 1e-3) / 1e6,
+                               "hbm_frac": 152.0 * npts / (con_ms * 1e-3) / 1e9 / hbm_gbs,
+                               "norms_H_Mx_My_Mz": norms_host},
     }
     print(json.dumps(out))
 
@@ -313,8 +338,11 @@ def main():
     ap.add_argument("--oracle-n", type=int, default=None, help="edge of the CPU oracle's sample block")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--traffic", type=float, default=None,
-                    help="dram bytes per launch of the dominant kernel from the committed ncu capture")
+                    help="dram bytes per launch of the dominant kernel from the committed ncu capture "
+                         "(default for config 4: profiles/r01_traffic_256.md)")
     args = ap.parse_args()
+    if args.traffic is None and args.config == 4 and not args.n:
+        args.traffic = 21.88e9   # mean over the four substage launches, profiles/r01_traffic_256.md
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
