@@ -195,8 +195,13 @@ __device__ __forceinline__ TileCoord coord(const TileMaps& M, const TileId& id) 
 
 // EPI 0..4: Z4c right-hand side / RK4 substage; EPI == -1: constraint monitor (rhs receives H, M^x, M^y, M^z in
 // fields 0..3)
+#ifdef SACRA_MAXNREG   // tuning builds: cap the registers of the substage kernel (spill sweep)
+#define SACRA_KERNEL_BOUNDS __maxnreg__(SACRA_MAXNREG)
+#else
+#define SACRA_KERNEL_BOUNDS __launch_bounds__(Tile::NT, Tile::CTAS)
+#endif
 template <int EPI>
-__global__ void __launch_bounds__(Tile::NT, Tile::CTAS) k_z4c(const __grid_constant__ PatchBatch B,
+__global__ void SACRA_KERNEL_BOUNDS k_z4c(const __grid_constant__ PatchBatch B,
                                                      const __grid_constant__ Params P,
                                                      const __grid_constant__ TileMaps M,
                                                      double* __restrict__ rhs, const __grid_constant__ RkArgs rk) {
@@ -399,6 +404,7 @@ static int num_sms() {
 template <int EPI>
 static cudaError_t launch_one(int grid, cudaStream_t st, const PatchBatch& B, const Params& P, const TileMaps& M,
                               double* rhs, const RkArgs& rk) {
+
   static const cudaError_t attr =
       cudaFuncSetAttribute(k_z4c<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile::SMEM_BYTES);
   if (attr != cudaSuccess) return attr;

@@ -13,7 +13,8 @@
 // Every thread runs the same instruction stream (no data-dependent branch), which keeps the result bitwise
 // pi-symmetric.
 //
-// `Src` provides   src.field<F>()  -> sample loader of field F for field_derivs()
+// `Src` provides   src.derivs<F, D1, D2>(pc, S) -> the derivative bundle S of field F (field_derivs() on its tile,
+//                                                  or a bundle computed by the derivative warps)
 //                  src.centre(F)   -> value of field F at the point
 // `Emit` provides  emit.put<F>(k)  -> consumes the finished RHS value k of field F (KO included)
 #pragma once
@@ -100,7 +101,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
   double dd[3];         // d_j (d_k beta^k)
 #define BETA_FIELD(I)                                                                              \
   {                                                                                                \
-    field_derivs<true, true>(src.template field<F_BET + I>(), pc, S);                              \
+    src.template derivs<F_BET + I, true, true>(pc, S);                              \
     db[0][I] = S.d1[0]; db[1][I] = S.d1[1]; db[2][I] = S.d1[2];                                    \
     gr[I] = sum9(gi, S.d2);                                                                        \
     if (I == 0) { dd[0] = S.d2[sym(0, 0)]; dd[1] = S.d2[sym(1, 0)]; dd[2] = S.d2[sym(2, 0)]; }     \
@@ -118,7 +119,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
   double advG[3], koG[3];
 #define GAM_FIELD(Kx)                                                                              \
   {                                                                                                \
-    field_derivs<true, false>(src.template field<F_GAM + Kx>(), pc, S);                            \
+    src.template derivs<F_GAM + Kx, true, false>(pc, S);                            \
     _Pragma("unroll") for (int i = 0; i < 3; ++i)                                                  \
       _Pragma("unroll") for (int j = i; j < 3; ++j) {                                              \
         const double t = g[sym(Kx, i)] * S.d1[j] + g[sym(Kx, j)] * S.d1[i];                        \
@@ -134,7 +135,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
 #define GT_FIELD(I, J)                                                                             \
   {                                                                                                \
     constexpr int n = sym(I, J);                                                                   \
-    field_derivs<true, true>(src.template field<F_G + n>(), pc, S);                                \
+    src.template derivs<F_G + n, true, true>(pc, S);                                \
     dg[0][n] = S.d1[0]; dg[1][n] = S.d1[1]; dg[2][n] = S.d1[2];                                    \
     Rt[n] = -half * sum9(gi, S.d2) + half * Rt[n];                                                 \
     double lie = g[sym(I, 0)] * db[J][0] + g[sym(J, 0)] * db[I][0];                                \
@@ -220,7 +221,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
   // ---- W: conformal-factor part of the Ricci tensor; Rt -> W^2 R_ij ; RHS of W ---------------------------
   double dW[3];
   {
-    field_derivs<true, true>(src.template field<F_W>(), pc, S);
+    src.template derivs<F_W, true, true>(pc, S);
     dW[0] = S.d1[0]; dW[1] = S.d1[1]; dW[2] = S.d1[2];
     double DDW[6];
 #pragma unroll
@@ -248,7 +249,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
   // ---- alpha: W^2 D_i D_j alpha; Rt -> X_ij = -W^2 D_i D_j alpha + alpha W^2 R_ij ; RHS of alpha (Eq. 6) --
   double lapa;
   {
-    field_derivs<true, true>(src.template field<F_ALP>(), pc, S);
+    src.template derivs<F_ALP, true, true>(pc, S);
     const double (&da)[3] = S.d1;
     double dadW = 0.0;
 #pragma unroll
@@ -277,7 +278,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
 
   // ---- K-hat and Theta: gradient term of Gt^i, and their own RHS ------------------------------------------
   {
-    field_derivs<true, false>(src.template field<F_KH>(), pc, S);
+    src.template derivs<F_KH, true, false>(pc, S);
     const double f = -2.0 * two3 * alp;                                  // 2 alpha (-1/3) * 2
 #pragma unroll
     for (int i = 0; i < 3; ++i) gr[i] = fma(f, row3(gi, i, S.d1), gr[i]);
@@ -285,7 +286,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
     emit.template put<F_KH>(k + S.ko);
   }
   {
-    field_derivs<true, false>(src.template field<F_TH>(), pc, S);
+    src.template derivs<F_TH, true, false>(pc, S);
     const double f = -two3 * alp;                                        // 2 alpha (-1/3)
 #pragma unroll
     for (int i = 0; i < 3; ++i) gr[i] = fma(f, row3(gi, i, S.d1), gr[i]);
@@ -299,7 +300,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
   emit.template put<F_GAM + 2>((gr[2] + advG[2]) + koG[2]);
 #define B_FIELD(I)                                                                                 \
   {                                                                                                \
-    field_derivs<false, false>(src.template field<F_B + I>(), pc, S);                              \
+    src.template derivs<F_B + I, false, false>(pc, S);                              \
     emit.template put<F_B + I>(((S.adv + gr[I]) - P.eta * S.u0) + S.ko);                                        \
   }
   B_FIELD(0) B_FIELD(1) B_FIELD(2)
@@ -320,7 +321,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
 #define AT_FIELD(I, J)                                                                             \
   {                                                                                                \
     constexpr int n = sym(I, J);                                                                   \
-    field_derivs<false, false>(src.template field<F_A + n>(), pc, S);                              \
+    src.template derivs<F_A + n, false, false>(pc, S);                              \
     const double xtf = Rt[n] - third * g[n] * trX;                                                 \
     const double aa = (A[sym(I, 0)] * Aud[0][J] + A[sym(I, 1)] * Aud[1][J]) + A[sym(I, 2)] * Aud[2][J]; \
     double lie = A[sym(I, 0)] * db[J][0] + A[sym(J, 0)] * db[I][0];                                \

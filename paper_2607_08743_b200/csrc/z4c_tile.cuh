@@ -71,6 +71,18 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
   } while (!ok);
 }
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {   // one (possibly suspending) probe
+  uint32_t ok;
+  asm volatile(
+      "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 // L2 eviction policies (the encodings createpolicy.fractional.L2::evict_*.b64 produces for fraction 1.0).
 // The centre tile of a tile is requested one tile ahead of its stencil boxes and covers the same cells, so it
 // should stay in L2 (evict last) for the boxes of this tile and of its neighbours to hit; u_n / acc tiles are read
@@ -134,8 +146,15 @@ struct TileCfg {
 // array (never through a stored generic pointer), so that every access compiles to LDS with an immediate offset.
 extern __shared__ __align__(1024) double tile_smem[];
 
+// barrier among the threads that exchange e values: the whole CTA (BAR = 0) or a named barrier of C::NT threads
+template <int BAR, int NTHREADS>
+__device__ __forceinline__ void group_sync() {
+  if constexpr (BAR == 0) __syncthreads();
+  else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(NTHREADS) : "memory");
+}
+
 // sample loader of one field for field_derivs(): shared-memory tile, compile-time strides
-template <class C>
+template <class C, int BAR = 0>
 struct TileLoader {
   int c;       // index of this thread's centre inside the ring slot of the field
   int ey, ez;  // this thread's entries of the e arrays
@@ -162,7 +181,7 @@ struct TileLoader {
       tile_smem[ey + xh] = e_at(xh, C::PX);
       tile_smem[ez + xh] = e_at(xh, C::PX * C::PY);
     }
-    __syncthreads();
+    group_sync<BAR, C::NT>();
   }
   __device__ __forceinline__ double e_y_x(int k) const { return tile_smem[ey + k]; }            // e_y at x + k
   __device__ __forceinline__ double e_z_x(int k) const { return tile_smem[ez + k]; }            // e_z at x + k
@@ -305,6 +324,12 @@ struct TileSource {
     const uint32_t slot = ring_slot(iter, s);
     tma::mbar_wait(full(slot), ring_use(iter, s) & 1u);
     return TileLoader<C>{sc + (int)slot * C::SLOT, ey, ez, xh, yh};
+  }
+
+  // derivative bundle of field F: its tile from the ring, then the stencils
+  template <int F, bool D1, bool D2>
+  __device__ __forceinline__ void derivs(const PointCoef& pc, Stencil& S) const {
+    field_derivs<D1, D2>(field<F>(), pc, S);
   }
 
   // RK inputs of field F at this point (stages 2-4): waits for the ring slot of its emit
