@@ -7,9 +7,10 @@
 // Order of the fields:
 //     beta^i -> Gt^i -> gt_ij -> (Christoffels) -> W -> alpha -> K-hat -> Theta -> (Gt^i out) -> B^i -> At_ij
 //
-// Numerics policy: -fmad=false; every sum is written in index order, one
-// rounding per operation, with two deliberate exceptions that use FMA chains and a regrouped contraction:
-// the quadratic Christoffel block of the conformal Ricci tensor and the running sum of the Gt^i RHS.
+// Numerics policy: -fmad=false. The RHS of the O(1) fields (W, gt_ij, alpha, beta^i) is
+// assembled in the oracle's index order, one rounding per operation. Blocks that only feed K-hat, Theta, At_ij,
+// Gt^i, B^i use FMA chains and regrouped contractions: the symmetric contractions gi^lm t_lm, the quadratic
+// Christoffel block of the conformal Ricci tensor and the running sum of the Gt^i RHS.
 // Every thread runs the same instruction stream (no data-dependent branch), which keeps the result bitwise
 // pi-symmetric.
 //
@@ -27,12 +28,13 @@ struct Params {        // device copy of sacra_params_t
   int lapse_uses_khat;
 };
 
-// full double sum over (l,m) in row-major order of gi^lm t_lm, both symmetric (packed); the six distinct
-// products are formed once, the nine additions are done in index order.
+// contraction gi^lm t_lm of two symmetric tensors (packed): diagonal + 2 x off-diagonal, FMA chains. Every use
+// feeds the RHS of K-hat, Theta, At_ij or Gt^i only -- fields whose state is << 1, where a last-bit difference from
+// the oracle's index-order sum cannot flip the rounding of an O(1) stage input.
 __device__ __forceinline__ double sum9(const double (&gi)[6], const double (&t)[6]) {
-  const double p00 = gi[0] * t[0], p01 = gi[1] * t[1], p02 = gi[2] * t[2];
-  const double p11 = gi[3] * t[3], p12 = gi[4] * t[4], p22 = gi[5] * t[5];
-  return (((((((p00 + p01) + p02) + p01) + p11) + p12) + p02) + p12) + p22;
+  const double d = fma(gi[5], t[5], fma(gi[3], t[3], gi[0] * t[0]));
+  const double o = fma(gi[4], t[4], fma(gi[2], t[2], gi[1] * t[1]));
+  return fma(2.0, o, d);
 }
 // sum_j m[i][j] v[j] in index order, m symmetric packed
 __device__ __forceinline__ double row3(const double (&m)[6], int i, const double (&v)[3]) {
