@@ -90,11 +90,11 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
 #pragma unroll
       for (int j = 0; j < 3; ++j)
         Auu[i][j] = (Aud[i][0] * gi[sym(0, j)] + Aud[i][1] * gi[sym(1, j)]) + Aud[i][2] * gi[sym(2, j)];
-    AA = 0.0;
-#pragma unroll
-    for (int i = 0; i < 3; ++i)
-#pragma unroll
-      for (int j = 0; j < 3; ++j) AA += A[sym(i, j)] * Auu[i][j];
+    {   // At_ij At^ij: diagonal + the two index orders of the off-diagonal pairs, FMA tree (feeds K-hat, Theta only)
+      const double d = fma(A[5], Auu[2][2], fma(A[3], Auu[1][1], A[0] * Auu[0][0]));
+      const double o = fma(A[4], Auu[1][2] + Auu[2][1], fma(A[2], Auu[0][2] + Auu[2][0], A[1] * (Auu[0][1] + Auu[1][0])));
+      AA = d + o;
+    }
   }
 
   // ---- beta^i: d_k beta^i; gt^jk d_j d_k beta^i; d_j d_k beta^k; RHS of beta^i (Eq. 7) -------------------
@@ -225,17 +225,14 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
   {
     src.template derivs<F_W, true, true>(pc, S);
     dW[0] = S.d1[0]; dW[1] = S.d1[1]; dW[2] = S.d1[2];
-    double DDW[6];
+    double DDW[6], dW2[6];   // Dt_i Dt_j W and d_i W d_j W (both only feed the Ricci tensor: FMA chains)
 #pragma unroll
-    for (int n = 0; n < 6; ++n) DDW[n] = ((S.d2[n] - Gu[0][n] * dW[0]) - Gu[1][n] * dW[1]) - Gu[2][n] * dW[2];
-    double trDDW = 0.0, dWdW = 0.0;
+    for (int n = 0; n < 6; ++n) DDW[n] = fma(-Gu[2][n], dW[2], fma(-Gu[1][n], dW[1], fma(-Gu[0][n], dW[0], S.d2[n])));
 #pragma unroll
-    for (int k = 0; k < 3; ++k)
+    for (int i = 0; i < 3; ++i)
 #pragma unroll
-      for (int l = 0; l < 3; ++l) {
-        trDDW += gi[sym(k, l)] * DDW[sym(k, l)];
-        dWdW += gi[sym(k, l)] * dW[k] * dW[l];
-      }
+      for (int j = i; j < 3; ++j) dW2[sym(i, j)] = dW[i] * dW[j];
+    const double trDDW = sum9(gi, DDW), dWdW = sum9(gi, dW2);
 #pragma unroll
     for (int n = 0; n < 6; ++n)
       Rt[n] = W * W * Rt[n] + (W * (DDW[n] + g[n] * trDDW) - 2.0 * g[n] * dWdW);
@@ -253,18 +250,14 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
   {
     src.template derivs<F_ALP, true, true>(pc, S);
     const double (&da)[3] = S.d1;
-    double dadW = 0.0;
-#pragma unroll
-    for (int k = 0; k < 3; ++k)
-#pragma unroll
-      for (int l = 0; l < 3; ++l) dadW += gi[sym(k, l)] * da[k] * dW[l];
+    const double dadW = fma(da[2], row3(gi, 2, dW), fma(da[1], row3(gi, 1, dW), da[0] * row3(gi, 0, dW)));
     double WDDa[6];
 #pragma unroll
     for (int i = 0; i < 3; ++i)
 #pragma unroll
       for (int j = i; j < 3; ++j) {
         const int n = sym(i, j);
-        const double cov = ((S.d2[n] - Gu[0][n] * da[0]) - Gu[1][n] * da[1]) - Gu[2][n] * da[2];
+        const double cov = fma(-Gu[2][n], da[2], fma(-Gu[1][n], da[1], fma(-Gu[0][n], da[0], S.d2[n])));
         WDDa[n] = W * W * cov + W * ((da[i] * dW[j] + da[j] * dW[i]) - g[n] * dadW);
       }
     lapa = sum9(gi, WDDa);
