@@ -77,6 +77,17 @@ typedef struct {
  * padding beyond nx+2ng is not touched. */
 int sacra_fill_ghosts(const sacra_patch_t* p, int npatch, double* u, void* cuda_stream);
 
+/* Halo fill with a boundary mode per axis (axis_mode: HOST int32_t[3], x y z), SURVEY 8(f) f-2:
+ *   SACRA_BC_PERIODIC  as sacra_fill_ghosts;
+ *   SACRA_BC_MIRROR    reflection symmetry about both faces of the axis (PAPER.md:125 imposes it at z = 0): the ghost
+ *                      cell m+1 cells outside a face takes the active cell m cells inside it, times the parity of the
+ *                      field under x^a -> -x^a: -1 for Gt^a, beta^a, B^a and for the gt / At components with exactly
+ *                      one index a, +1 otherwise; cells reflected along several axes take the product.
+ * In place on u; all patches of the call use the same modes. */
+#define SACRA_BC_PERIODIC 0
+#define SACRA_BC_MIRROR 1
+int sacra_fill_ghosts_bc(const sacra_patch_t* p, int npatch, const int32_t* axis_mode, double* u, void* cuda_stream);
+
 /* Z4c right-hand side including KO dissipation, F(u) (PAPER.md:49-73,
  * PAPER.md:99). u: ghosts already filled (read only). rhs: the 25 RHS values are written on active cells;
  * ghost cells and padding of rhs are not touched. rhs must not alias u. */

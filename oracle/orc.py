@@ -152,3 +152,10 @@ def constraints_point(u, d1, d2):
     out = np.zeros(4)
     lib().orc_constraints_point(_p(u), _p(d1), _p(d2), _p(out))
     return out
+
+
+def fill_ghosts_bc(ps, mode, u):
+    """ghost fill with per-axis mode (0 periodic, 1 mirror with field parity), in place; mode = (mx, my, mz)"""
+    m = (C.c_int32 * 3)(*[int(v) for v in mode])
+    lib().orc_fill_ghosts_bc(_patches(ps), len(ps), m, _p(u))
+    return u

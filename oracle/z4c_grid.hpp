@@ -36,6 +36,52 @@ template <class T> void fill_ghosts(const Patch& p, T* state) {
   }
 }
 
+// SURVEY.md 8(f) row f-2 (first half): reflection symmetry as a ghost-fill mode ("we impose reflection
+// symmetry with respect to the equatorial plane z = 0"). Per axis a the mode is 0 = periodic (item 2) or 1 = mirror:
+// the ghost cell at distance m+1 outside a face takes the value of the active cell at distance m inside it
+// (cell-centred grid: the face lies half a cell outside the first active cell), times the parity of the field
+// under x^a -> -x^a: -1 for the a-component of a vector (Gt^a, beta^a, B^a) and for tensor components with exactly
+// one index a (gt, At), +1 otherwise. A corner cell reflected along several axes takes the product.
+inline int field_parity(int f, int axis) {
+  auto vec = [&](int f0) { return f >= f0 && f < f0 + 3 ? (f - f0 == axis ? -1 : 1) : 0; };
+  auto ten = [&](int f0) {
+    if (f < f0 || f >= f0 + 6) return 0;
+    static const int IJ[6][2] = {{0, 0}, {0, 1}, {0, 2}, {1, 1}, {1, 2}, {2, 2}};
+    const int n = (IJ[f - f0][0] == axis) + (IJ[f - f0][1] == axis);
+    return n == 1 ? -1 : 1;
+  };
+  if (int s = vec(F_GAM)) return s;
+  if (int s = vec(F_BET)) return s;
+  if (int s = vec(F_B)) return s;
+  if (int s = ten(F_G)) return s;
+  if (int s = ten(F_A)) return s;
+  return 1;   // W, K-hat, Theta, alpha
+}
+template <class T> void fill_ghosts_bc(const Patch& p, const int mode[3], T* state) {
+  const int sx = p.nx + 2 * NG, sy = p.ny + 2 * NG, sz = p.nz + 2 * NG;
+  const int nn[3] = {p.nx, p.ny, p.nz};
+  for (int n = 0; n < NF; ++n) {
+    T* f = state + p.offset + (long)n * p.fstride;
+#pragma omp parallel for schedule(static)
+    for (int Kk = 0; Kk < sz; ++Kk)
+      for (int J = 0; J < sy; ++J)
+        for (int I = 0; I < sx; ++I) {
+          const int S[3] = {I, J, Kk};
+          int src[3], sign = 1;
+          bool ghost = false;
+          for (int a = 0; a < 3; ++a) {
+            const int i = S[a] - NG;
+            if (i >= 0 && i < nn[a]) { src[a] = i; continue; }
+            ghost = true;
+            if (mode[a] == 0) src[a] = wrap(i, nn[a]);
+            else { src[a] = i < 0 ? -1 - i : 2 * nn[a] - 1 - i; sign *= field_parity(n, a); }
+          }
+          if (!ghost) continue;
+          f[cell(p, I, J, Kk)] = T(sign) * f[cell(p, src[0] + NG, src[1] + NG, src[2] + NG)];
+        }
+  }
+}
+
 // items 3-10 on every active cell. u is ghost-filled; rhs is written on active
 // cells only (ghosts untouched).
 template <class T>

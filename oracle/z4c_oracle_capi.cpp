@@ -58,6 +58,10 @@ void orc_set_threads(int n) { omp_set_num_threads(n); }
 void orc_fill_ghosts(const orc_patch* ps, int np, double* u) {
   for (int q = 0; q < np; ++q) fill_ghosts<double>(to_patch(ps[q]), u);
 }
+void orc_fill_ghosts_bc(const orc_patch* ps, int np, const int32_t* mode, double* u) {
+  const int m[3] = {mode[0], mode[1], mode[2]};
+  for (int q = 0; q < np; ++q) fill_ghosts_bc<double>(to_patch(ps[q]), m, u);
+}
 void orc_z4c_rhs(const orc_patch* ps, int np, const orc_params* prm, const double* u, double* rhs) {
   auto P = to_params<double>(*prm);
   for (int q = 0; q < np; ++q) rhs_patch<double>(to_patch(ps[q]), P, u, rhs);

@@ -32,10 +32,39 @@ struct PatchBatch {
 };
 
 // ---------------------------------------------------------------------------------------------------
-// Periodic halo fill. Only ghost cells are written and only active cells are read (every source index is
-// wrapped into the active range), so reads and writes never overlap: item 2.
+// Halo fill. Per axis: periodic (item 2; stands in for the paper's ghost exchange) or mirror (SURVEY 8(f) f-2,
+// reflection symmetry about a face; the value comes with the parity of the field under x^a -> -x^a).
+// Only ghost cells are written and only active cells are read (every source index is mapped into the active range),
+// so reads and writes never overlap.
 // ---------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ PatchBatch B, double* __restrict__ u) {
+struct FillMode {
+  int m[3];   // per axis: 0 periodic, 1 mirror
+};
+// -1 for the a-component of a vector and for tensor components with exactly one index a
+__device__ __forceinline__ double field_parity(int f, int axis) {
+  if (f >= F_GAM && f < F_GAM + 3) return f - F_GAM == axis ? -1.0 : 1.0;
+  if (f >= F_BET && f < F_BET + 3) return f - F_BET == axis ? -1.0 : 1.0;
+  if (f >= F_B && f < F_B + 3) return f - F_B == axis ? -1.0 : 1.0;
+  int n = -1;
+  if (f >= F_G && f < F_G + 6) n = f - F_G;
+  if (f >= F_A && f < F_A + 6) n = f - F_A;
+  if (n < 0) return 1.0;
+  // packed xx xy xz yy yz zz: components with exactly one index equal to `axis`
+  const int one[3] = {0b000110, 0b010010, 0b010100};   // x: xy xz | y: xy yz | z: xz yz
+  return (one[axis] >> n) & 1 ? -1.0 : 1.0;
+}
+// storage index of the source cell of storage index I along an axis with n active cells; *refl: a mirror was used
+__device__ __forceinline__ int fill_source(int I, int n, int mode, bool* refl) {
+  const int i = I - NG;
+  *refl = false;
+  if (i >= 0 && i < n) return I;
+  if (mode == 0) return (i < 0 ? i + n : i - n) + NG;
+  *refl = true;
+  return (i < 0 ? -1 - i : 2 * n - 1 - i) + NG;
+}
+
+__global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ PatchBatch B, const __grid_constant__ FillMode mode,
+                                                     double* __restrict__ u) {
   int ip = 0;
 #pragma unroll 1
   while (ip + 1 < B.np && (int)blockIdx.x >= B.first_block[ip + 1]) ++ip;
@@ -43,30 +72,32 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
   const int sx = p.nx + 2 * NG, sy = p.ny + 2 * NG;
   // one block = one storage plane K of one field: a ghost plane is copied whole, an active plane only
   // has its 6 ghost rows and the 3+3 x-ghosts of its active rows
+  const int f = blockIdx.y;
   const int Kk = (int)blockIdx.x - B.first_block[ip];
-  int k = Kk - NG;
-  const bool plane_ghost = (k < 0) | (k >= p.nz);
-  k = k < 0 ? k + p.nz : (k >= p.nz ? k - p.nz : k);
-  double* fld = u + p.offset + (long long)blockIdx.y * p.fstride;
+  bool rz, ry, rx;
+  const int Ks = fill_source(Kk, p.nz, mode.m[2], &rz);
+  const bool plane_ghost = Ks != Kk;
+  const double pz = rz ? field_parity(f, 2) : 1.0, py = field_parity(f, 1), px = field_parity(f, 0);
+  double* fld = u + p.offset + (long long)f * p.fstride;
   double* dst = fld + (long long)Kk * p.sz;
-  const double* src = fld + (long long)(k + NG) * p.sz;
-  auto wrapx = [&](int I) { int i = I - NG; i = i < 0 ? i + p.nx : (i >= p.nx ? i - p.nx : i); return i + NG; };
-  auto wrapy = [&](int J) { int j = J - NG; j = j < 0 ? j + p.ny : (j >= p.ny ? j - p.ny : j); return j + NG; };
+  const double* src = fld + (long long)Ks * p.sz;
+  auto copy_row = [&](int J) {   // one warp: the whole storage row J of this plane
+    const int Js = fill_source(J, p.ny, mode.m[1], &ry);
+    const double s = pz * (ry ? py : 1.0);
+    for (int I = threadIdx.x % 32; I < sx; I += 32) {
+      const int Is = fill_source(I, p.nx, mode.m[0], &rx);
+      dst[(long long)J * p.pitch + I] = (rx ? s * px : s) * src[(long long)Js * p.pitch + Is];
+    }
+  };
   if (plane_ghost) {
-    for (int J = threadIdx.x / 32; J < sy; J += blockDim.x / 32) {     // one warp per row
-      const long long sr = (long long)wrapy(J) * p.pitch, dr = (long long)J * p.pitch;
-      for (int I = threadIdx.x % 32; I < sx; I += 32) dst[dr + I] = src[sr + wrapx(I)];
-    }
+    for (int J = threadIdx.x / 32; J < sy; J += blockDim.x / 32) copy_row(J);
   } else {
-    for (int r = threadIdx.x / 32; r < 2 * NG; r += blockDim.x / 32) {  // ghost rows 0..2, ny+3..ny+5
-      const int J = r < NG ? r : p.ny + r;
-      const long long sr = (long long)wrapy(J) * p.pitch, dr = (long long)J * p.pitch;
-      for (int I = threadIdx.x % 32; I < sx; I += 32) dst[dr + I] = src[sr + wrapx(I)];
-    }
+    for (int r = threadIdx.x / 32; r < 2 * NG; r += blockDim.x / 32) copy_row(r < NG ? r : p.ny + r);   // ghost rows
     for (int q = threadIdx.x; q < p.ny * 2 * NG; q += blockDim.x) {     // x-ghosts of the active rows
       const int J = q / (2 * NG) + NG, c = q % (2 * NG);
       const int I = c < NG ? c : p.nx + c;
-      dst[(long long)J * p.pitch + I] = src[(long long)J * p.pitch + wrapx(I)];
+      const int Is = fill_source(I, p.nx, mode.m[0], &rx);
+      dst[(long long)J * p.pitch + I] = (rx ? px : 1.0) * src[(long long)J * p.pitch + Is];
     }
   }
 }
@@ -339,7 +370,8 @@ static Params to_dev(const sacra_params_t& a) {
   return P;
 }
 
-static int launch_fill(const sacra_patch_t* p, int npatch, double* u, cudaStream_t st) {
+static int launch_fill(const sacra_patch_t* p, int npatch, double* u, cudaStream_t st,
+                       FillMode mode = FillMode{{0, 0, 0}}) {
   for (int q0 = 0; q0 < npatch; q0 += MAXP) {
     PatchBatch B;
     B.np = (npatch - q0 < MAXP) ? npatch - q0 : MAXP;
@@ -350,7 +382,7 @@ static int launch_fill(const sacra_patch_t* p, int npatch, double* u, cudaStream
       nb += p[q0 + q].nz + 2 * NG;
     }
     B.first_block[B.np] = nb;
-    k_fill_ghosts<<<dim3(nb, NF), 256, 0, st>>>(B, u);
+    k_fill_ghosts<<<dim3(nb, NF), 256, 0, st>>>(B, mode, u);
     if (cudaGetLastError() != cudaSuccess) return SACRA_ERR_CUDA;
   }
   return SACRA_OK;
@@ -463,6 +495,18 @@ int sacra_fill_ghosts(const sacra_patch_t* p, int npatch, double* u, void* cuda_
   if (int e = check_patches(p, npatch)) return e;
   if (!aligned16(u)) return SACRA_ERR_ALIGN;
   return launch_fill(p, npatch, u, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int sacra_fill_ghosts_bc(const sacra_patch_t* p, int npatch, const int32_t* axis_mode, double* u, void* cuda_stream) {
+  if (!p || !u || !axis_mode) return SACRA_ERR_NULL;
+  if (int e = check_patches(p, npatch)) return e;
+  if (!aligned16(u)) return SACRA_ERR_ALIGN;
+  FillMode m;
+  for (int a = 0; a < 3; ++a) {
+    if (axis_mode[a] != SACRA_BC_PERIODIC && axis_mode[a] != SACRA_BC_MIRROR) return SACRA_ERR_BADARG;
+    m.m[a] = axis_mode[a];
+  }
+  return launch_fill(p, npatch, u, static_cast<cudaStream_t>(cuda_stream), m);
 }
 
 int sacra_z4c_rhs(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, const double* u, double* rhs,

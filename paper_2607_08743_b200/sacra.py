@@ -19,7 +19,8 @@ NG = 3
 OK, ERR_NULL, ERR_BADARG, ERR_UNSUPPORTED, ERR_ALIGN, ERR_CUDA = 0, -1, -2, -3, -4, -5
 EXPORTS = ("sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4_step",
            "sacra_strerror", "sacra_version",
-           "sacra_constraints", "sacra_constraint_norms", "sacra_constraint_scratch_doubles")
+           "sacra_constraints", "sacra_constraint_norms", "sacra_constraint_scratch_doubles",
+           "sacra_fill_ghosts_bc")
 
 
 class SacraPatch(C.Structure):
@@ -55,7 +56,8 @@ def _load():
     lib.sacra_constraint_norms.argtypes = [vp, i32, dp, dp, dp, vp]
     lib.sacra_constraint_scratch_doubles.argtypes = [vp, i32]
     lib.sacra_constraint_scratch_doubles.restype = C.c_int64
-    for n in EXPORTS[:4] + EXPORTS[6:8]:
+    lib.sacra_fill_ghosts_bc.argtypes = [vp, i32, vp, dp, vp]
+    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:10]:
         getattr(lib, n).restype = C.c_int
     lib.sacra_strerror.argtypes = [C.c_int]
     lib.sacra_strerror.restype = C.c_char_p
@@ -165,3 +167,13 @@ def constraint_norms(patches, con, scratch, norms, stream=None):
     ps = make_patches(patches) if patches is not None else None
     _check(lib.sacra_constraint_norms(ps, len(ps) if ps is not None else 0, _ptr(con), _ptr(scratch), _ptr(norms),
                                       _stream(stream)))
+
+
+BC_PERIODIC, BC_MIRROR = 0, 1
+
+
+def fill_ghosts_bc(patches, axis_mode, u, stream=None):
+    """halo fill with a mode per axis (BC_PERIODIC / BC_MIRROR for x, y, z)"""
+    ps = make_patches(patches) if patches is not None else None
+    m = (C.c_int32 * 3)(*[int(v) for v in axis_mode])
+    _check(lib.sacra_fill_ghosts_bc(ps, len(ps) if ps is not None else 0, m, _ptr(u), _stream(stream)))
