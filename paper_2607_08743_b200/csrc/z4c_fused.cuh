@@ -74,28 +74,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
   const double W = src.centre(F_W), alp = src.centre(F_ALP), Kh = src.centre(F_KH), Th = src.centre(F_TH);
   const double K = Kh + 2.0 * Th;                                        // item 7: K = K-hat + 2 Theta
 
-  // At^i_j, At^ij (all nine: the two index orders round differently) and At_ij At^ij
-  double Auu[3][3], AA;
-  {
-    double A[6], Aud[3][3];
-#pragma unroll
-    for (int n = 0; n < 6; ++n) A[n] = src.centre(F_A + n);
-#pragma unroll
-    for (int i = 0; i < 3; ++i)
-#pragma unroll
-      for (int j = 0; j < 3; ++j)
-        Aud[i][j] = (gi[sym(i, 0)] * A[sym(0, j)] + gi[sym(i, 1)] * A[sym(1, j)]) + gi[sym(i, 2)] * A[sym(2, j)];
-#pragma unroll
-    for (int i = 0; i < 3; ++i)
-#pragma unroll
-      for (int j = 0; j < 3; ++j)
-        Auu[i][j] = (Aud[i][0] * gi[sym(0, j)] + Aud[i][1] * gi[sym(1, j)]) + Aud[i][2] * gi[sym(2, j)];
-    {   // At_ij At^ij: diagonal + the two index orders of the off-diagonal pairs, FMA tree (feeds K-hat, Theta only)
-      const double d = fma(A[5], Auu[2][2], fma(A[3], Auu[1][1], A[0] * Auu[0][0]));
-      const double o = fma(A[4], Auu[1][2] + Auu[2][1], fma(A[2], Auu[0][2] + Auu[2][0], A[1] * (Auu[0][1] + Auu[1][0])));
-      AA = d + o;
-    }
-  }
+  double Auu[3][3], AA;   // At^ij and At_ij At^ij: formed at the Christoffel block, where they are first needed
 
   // ---- beta^i: d_k beta^i; gt^jk d_j d_k beta^i; d_j d_k beta^k; RHS of beta^i (Eq. 7) -------------------
   double db[3][3];      // db[k][i] = d_k beta^i
@@ -171,7 +150,16 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
     //        + gt^lm ( Gt^k_li Gt_jkm + Gt^k_lj Gt_ikm + Gt^k_im Gt_klj )            [relaxed, regrouped:]
     // with H_i[k][m] = gt^lm Gt^k_li :  T1_ij = H_i[k][m] Gt_jkm ,  T3_ij = H_i[k][l] Gt_klj ,
     // quadratic block = T1_ij + T1_ji + T3_ij.
-    double T1[3][3], T3[6];
+    // Every piece is added to Rt_ij as soon as it exists (no T1 / T3 arrays: 15 fewer live values at the register
+    // peak of the kernel); the diagonal takes T1_ii twice.
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int j = i; j < 3; ++j) {
+        const double t3 = fma(Gd[2], Gl[i][sym(j, 2)] + Gl[j][sym(i, 2)],
+                              fma(Gd[1], Gl[i][sym(j, 1)] + Gl[j][sym(i, 1)], Gd[0] * (Gl[i][sym(j, 0)] + Gl[j][sym(i, 0)])));
+        Rt[sym(i, j)] = fma(half, t3, Rt[sym(i, j)]);
+      }
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
       double H[3][3];
@@ -182,27 +170,39 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
           H[k][m] = fma(gi[sym(2, m)], Gu[k][sym(2, i)], fma(gi[sym(1, m)], Gu[k][sym(1, i)], gi[sym(0, m)] * Gu[k][sym(0, i)]));
 #pragma unroll
       for (int j = 0; j < 3; ++j) {
-        double t = 0.0, t3 = 0.0;
+        // three partial chains per contraction (k = 0, 1, 2) instead of one chain of nine
+        double t[3], t3[3];
 #pragma unroll
-        for (int k = 0; k < 3; ++k)
-#pragma unroll
-          for (int m = 0; m < 3; ++m) {
-            t = fma(H[k][m], Gl[j][sym(k, m)], t);
-            if (j >= i) t3 = fma(H[k][m], Gl[k][sym(m, j)], t3);
-          }
-        T1[i][j] = t;
-        if (j >= i) T3[sym(i, j)] = t3;
+        for (int k = 0; k < 3; ++k) {
+          t[k] = fma(H[k][2], Gl[j][sym(k, 2)], fma(H[k][1], Gl[j][sym(k, 1)], H[k][0] * Gl[j][sym(k, 0)]));
+          if (j >= i) t3[k] = fma(H[k][2], Gl[k][sym(2, j)], fma(H[k][1], Gl[k][sym(1, j)], H[k][0] * Gl[k][sym(0, j)]));
+        }
+        const double T1 = (t[0] + t[1]) + t[2];
+        Rt[sym(i, j)] += (i == j) ? 2.0 * T1 : T1;
+        if (j >= i) Rt[sym(i, j)] += (t3[0] + t3[1]) + t3[2];
       }
     }
-#pragma unroll
-    for (int i = 0; i < 3; ++i)
-#pragma unroll
-      for (int j = i; j < 3; ++j) {
-        double t3 = Gd[0] * (Gl[i][sym(j, 0)] + Gl[j][sym(i, 0)]);
-        t3 += Gd[1] * (Gl[i][sym(j, 1)] + Gl[j][sym(i, 1)]);
-        t3 += Gd[2] * (Gl[i][sym(j, 2)] + Gl[j][sym(i, 2)]);
-        Rt[sym(i, j)] = (Rt[sym(i, j)] + half * t3) + ((T1[i][j] + T1[j][i]) + T3[sym(i, j)]);
+    // At^i_j, At^ij (all nine: the two index orders round differently) and At_ij At^ij
+    {
+      double A[6], Aud[3][3];
+  #pragma unroll
+      for (int n = 0; n < 6; ++n) A[n] = src.centre(F_A + n);
+  #pragma unroll
+      for (int i = 0; i < 3; ++i)
+  #pragma unroll
+        for (int j = 0; j < 3; ++j)
+          Aud[i][j] = (gi[sym(i, 0)] * A[sym(0, j)] + gi[sym(i, 1)] * A[sym(1, j)]) + gi[sym(i, 2)] * A[sym(2, j)];
+  #pragma unroll
+      for (int i = 0; i < 3; ++i)
+  #pragma unroll
+        for (int j = 0; j < 3; ++j)
+          Auu[i][j] = (Aud[i][0] * gi[sym(0, j)] + Aud[i][1] * gi[sym(1, j)]) + Aud[i][2] * gi[sym(2, j)];
+      {   // At_ij At^ij: diagonal + the two index orders of the off-diagonal pairs, FMA tree (feeds K-hat, Theta only)
+        const double d = fma(A[5], Auu[2][2], fma(A[3], Auu[1][1], A[0] * Auu[0][0]));
+        const double o = fma(A[4], Auu[1][2] + Auu[2][1], fma(A[2], Auu[0][2] + Auu[2][0], A[1] * (Auu[0][1] + Auu[1][0])));
+        AA = d + o;
       }
+    }
     // Gt^i RHS pieces that need the Christoffels                                      [relaxed running sum]
     //   2 alpha Gt^i_jk At^jk - Gt_d^j d_j beta^i + 2/3 Gt_d^i div beta - 2 alpha kappa1 (Gt^i - Gt_d^i)
 #pragma unroll
