@@ -11,6 +11,7 @@
 // the stencils has an immediate offset.
 #pragma once
 #include <cstdint>
+#include <type_traits>
 #include <cuda.h>   // CUtensorMap (types only; the encoder is fetched through cudaGetDriverEntryPoint)
 
 #include "z4c_stencil.cuh"
@@ -132,7 +133,11 @@ struct TileCfg {
   static constexpr int EX = TX + 4;                            // x extent of the e arrays (x halo of 2)
   static constexpr int EY_OFF = RK_OFF + RKD * 2 * NT;         // e_y on  TZ x TY x (TX+4)
   static constexpr int EZ_OFF = EY_OFF + TZ * TY * EX;         // e_z on  TZ x (TY+4) x (TX+4)
-  static constexpr int SMEM_BYTES = (EZ_OFF + TZ * (TY + 4) * EX) * 8;
+  static constexpr int ESZ = TZ * TY * EX + TZ * (TY + 4) * EX;   // one set of e arrays
+  // with room for a second set of e arrays, fields with mixed derivatives need one block barrier instead of two
+  // (MERGE: the ring refill waits for the barrier of the e exchange; the sets alternate)
+  static constexpr bool MERGE = (EY_OFF + 2 * ESZ) * 8 * CTAS + 1024 * CTAS <= 233472;
+  static constexpr int SMEM_BYTES = (EY_OFF + (MERGE ? 2 : 1) * ESZ) * 8;
   static_assert(SMEM_BYTES * CTAS + 1024 * CTAS <= 233472, "shared memory of the CTAs of one SM");
   static_assert(NF % RKD == 0 && NS + 2 + RKD <= 16, "mbarrier area / RK ring depth");
   static_assert(TY == 4 && TX >= 4, "e exchange: one y-halo row of e_z per thread row, x-halo columns by the edge lanes");
@@ -154,12 +159,13 @@ __device__ __forceinline__ void group_sync() {
 }
 
 // sample loader of one field for field_derivs(): shared-memory tile, compile-time strides
-template <class C, int BAR = 0>
+template <class C, int BAR = 0, class Owner = void, int S = -1>
 struct TileLoader {
   int c;       // index of this thread's centre inside the ring slot of the field
   int ey, ez;  // this thread's entries of the e arrays
   int xh;      // x-halo duty of this thread: 0 none, else the x offset (-2 or +2) of the column it also computes
   int yh;      // y offset (-2 or +2 rows... in units of rows) of the e_z y-halo entry this thread computes
+  const Owner* owner;   // MERGE: the tile source, told when the barrier of the e exchange has been passed
   __device__ __forceinline__ static constexpr int stride(int a) { return a == 0 ? 1 : (a == 1 ? C::PX : C::PX * C::PY); }
   __device__ __forceinline__ double operator()(int a, int k) const { return tile_smem[c + k * stride(a)]; }
   __device__ __forceinline__ double e_at(int o, int st) const {   // inner difference along stride st at centre + o
@@ -182,6 +188,7 @@ struct TileLoader {
       tile_smem[ez + xh] = e_at(xh, C::PX * C::PY);
     }
     group_sync<BAR, C::NT>();
+    if constexpr (!std::is_void<Owner>::value) owner->template after_publish<S>();
   }
   __device__ __forceinline__ double e_y_x(int k) const { return tile_smem[ey + k]; }            // e_y at x + k
   __device__ __forceinline__ double e_z_x(int k) const { return tile_smem[ez + k]; }            // e_z at x + k
@@ -306,24 +313,51 @@ struct TileSource {
     }
   }
 
+  // number of fields with mixed derivatives before stream position s (the e-array sets alternate between them)
+  __host__ __device__ static constexpr int d2_before(int s) {
+    int n = 0;
+    for (int q = 0; q < s; ++q) {
+      const int f = Stream::field(q);
+      if (f == F_W || (f >= F_G && f < F_G + 6) || f == F_ALP || (f >= F_BET && f < F_BET + 3)) ++n;
+    }
+    return n;
+  }
+  __host__ __device__ static constexpr bool is_d2(int f) {
+    return f == F_W || (f >= F_G && f < F_G + 6) || f == F_ALP || (f >= F_BET && f < F_BET + 3);
+  }
+  // leader: every thread is done with the slot of field s-1 and with every RK slot read so far -- refill them
+  template <int s>
+  __device__ __forceinline__ void refill() const {
+    issue<s + C::NS - 1>();
+    if constexpr (RK == 2) {
+      // emit e may be loaded once emit e - RKD is done: through emits_before(s) + RKD - 1
+      constexpr int hi = emits_before(s) + C::RKD - 1;
+      constexpr int lo = s == 0 ? C::RKD - 2 : emits_before(s - 1) + C::RKD - 1;
+      issue_rk_range<lo, hi>();
+    }
+  }
+  template <int s>
+  __device__ __forceinline__ void after_publish() const {
+    if (tid == 0) refill<s>();
+  }
+
   template <int F>
-  __device__ __forceinline__ TileLoader<C> field() const {
+  __device__ __forceinline__ auto field() const {
     constexpr int s = Stream::slot(F);
     static_assert(s >= 0, "field not in this kernel's stream");
-    // every thread is done with the slot of field s-1 and with every RK slot read so far: refill them
-    __syncthreads();
-    if (tid == 0) {
-      issue<s + C::NS - 1>();
-      if constexpr (RK == 2) {
-        // emit e may be loaded once emit e - RKD is done: through emits_before(s) + RKD - 1
-        constexpr int hi = emits_before(s) + C::RKD - 1;
-        constexpr int lo = s == 0 ? C::RKD - 2 : emits_before(s - 1) + C::RKD - 1;
-        issue_rk_range<lo, hi>();
-      }
+    constexpr bool merged = C::MERGE && is_d2(F);
+    if constexpr (!merged) {
+      __syncthreads();
+      if (tid == 0) refill<s>();
     }
     const uint32_t slot = ring_slot(iter, s);
     tma::mbar_wait(full(slot), ring_use(iter, s) & 1u);
-    return TileLoader<C>{sc + (int)slot * C::SLOT, ey, ez, xh, yh};
+    if constexpr (merged) {
+      constexpr int eo = (d2_before(s) & 1) * C::ESZ;
+      return TileLoader<C, 0, TileSource, s>{sc + (int)slot * C::SLOT, ey + eo, ez + eo, xh, yh, this};
+    } else {
+      return TileLoader<C>{sc + (int)slot * C::SLOT, ey, ez, xh, yh, nullptr};
+    }
   }
 
   // derivative bundle of field F: its tile from the ring, then the stencils

@@ -93,3 +93,17 @@ def test_alignment():
     assert _code(sacra.fill_ghosts, _patch(pitch_x=15)[0], FAKE) == sacra.ERR_ALIGN
     assert _code(sacra.fill_ghosts, _patch(patch_offset=4)[0], FAKE) == sacra.ERR_ALIGN    # offset+ng odd
     assert _code(sacra.z4c_rhs, ps, PRM, FAKE, FAKE + 8) == sacra.ERR_ALIGN
+
+
+def test_constraint_monitor_and_bc_fill_argument_checks():
+    ps, _ = _patch()
+    assert _code(sacra.constraints, ps, None, FAKE) == sacra.ERR_NULL
+    assert _code(sacra.constraints, ps, FAKE, FAKE) == sacra.ERR_BADARG            # con aliases u
+    assert _code(sacra.constraints, ps, FAKE, FAKE + 8) == sacra.ERR_ALIGN
+    assert _code(sacra.constraints, _patch(ng=2)[0], FAKE, FAKE + 64) == sacra.ERR_UNSUPPORTED
+    assert _code(sacra.constraint_norms, ps, FAKE, None, FAKE + 64) == sacra.ERR_NULL
+    assert _code(sacra.constraint_norms, ps, FAKE + 8, FAKE, FAKE + 64) == sacra.ERR_ALIGN
+    assert sacra.constraint_scratch_doubles(ps) == 4 * 8                            # 4 per active z-plane
+    assert _code(sacra.fill_ghosts_bc, ps, (0, 0, 2), FAKE) == sacra.ERR_BADARG     # unknown mode
+    assert _code(sacra.fill_ghosts_bc, ps, (0, 0, 1), None) == sacra.ERR_NULL
+    assert _code(sacra.fill_ghosts_bc, ps, (0, 1, 1), FAKE + 8) == sacra.ERR_ALIGN
