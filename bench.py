@@ -28,11 +28,11 @@ METRIC = "Z4c RHS+RK4 Mpoint-updates/s FP64"
 UNIT = "Mpoint-updates/s"
 NF = 25
 # Algorithmic work per point: 16 field passes x 8 B x 25 fields per RK4 step, i.e. 800 B per
-# substage launch on average; FP64 work per RHS evaluation + RK update after CSE: 3 586 FP64 instructions
-# (DADD 1 803, DMUL 921, DFMA 909 per point, ncu) = 4 542 flop with FMA = 2.
+# substage launch on average; FP64 work per RHS evaluation + RK update after CSE: 3 272 FP64 instructions
+# (DADD 1 401, DMUL 818, DFMA 1 053 per point in the SASS of k_z4c<2>) = 4 325 flop with FMA = 2.
 ALG_BYTES_PER_POINT_STEP = 16 * 8 * NF
-ALG_FLOP_PER_POINT_STAGE = 4542.0
-ALG_FP64_INSTR_PER_POINT_STAGE = 3586.0
+ALG_FLOP_PER_POINT_STAGE = 4325.0
+ALG_FP64_INSTR_PER_POINT_STAGE = 3272.0
 FP64_LANES_PER_SM, N_SM = 64, 148
 
 
