@@ -89,11 +89,14 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
       dst[(long long)J * p.pitch + I] = (rx ? s * px : s) * src[(long long)Js * p.pitch + Is];
     }
   };
+  // blockIdx.z splits the work of a plane: a whole ghost plane copied by one block is a chain of ~300 dependent
+  // DRAM round trips per warp (measured 0.31 ms per call at 256^3, all of it the six ghost planes)
+  const int nw = (blockDim.x / 32) * gridDim.z, w = (threadIdx.x / 32) * gridDim.z + blockIdx.z;   // warps of the plane
   if (plane_ghost) {
-    for (int J = threadIdx.x / 32; J < sy; J += blockDim.x / 32) copy_row(J);
+    for (int J = w; J < sy; J += nw) copy_row(J);
   } else {
-    for (int r = threadIdx.x / 32; r < 2 * NG; r += blockDim.x / 32) copy_row(r < NG ? r : p.ny + r);   // ghost rows
-    for (int q = threadIdx.x; q < p.ny * 2 * NG; q += blockDim.x) {     // x-ghosts of the active rows
+    for (int r = w; r < 2 * NG; r += nw) copy_row(r < NG ? r : p.ny + r);   // ghost rows
+    for (int q = threadIdx.x + blockDim.x * blockIdx.z; q < p.ny * 2 * NG; q += blockDim.x * gridDim.z) {   // x-ghosts
       const int J = q / (2 * NG) + NG, c = q % (2 * NG);
       const int I = c < NG ? c : p.nx + c;
       const int Is = fill_source(I, p.nx, mode.m[0], &rx);
@@ -375,14 +378,17 @@ static int launch_fill(const sacra_patch_t* p, int npatch, double* u, cudaStream
   for (int q0 = 0; q0 < npatch; q0 += MAXP) {
     PatchBatch B;
     B.np = (npatch - q0 < MAXP) ? npatch - q0 : MAXP;
-    int nb = 0;
+    int nb = 0, split = 1;
     for (int q = 0; q < B.np; ++q) {
       B.p[q] = to_dev(p[q0 + q]);
       B.first_block[q] = nb;
       nb += p[q0 + q].nz + 2 * NG;
+      const long long plane = (long long)(p[q0 + q].nx + 2 * NG) * (p[q0 + q].ny + 2 * NG);
+      const int want = plane / 8192 < 1 ? 1 : (plane / 8192 > 8 ? 8 : (int)(plane / 8192));
+      if (want > split) split = want;   // blocks per plane: only big planes are worth splitting
     }
     B.first_block[B.np] = nb;
-    k_fill_ghosts<<<dim3(nb, NF), 256, 0, st>>>(B, mode, u);
+    k_fill_ghosts<<<dim3(nb, NF, split), 256, 0, st>>>(B, mode, u);
     if (cudaGetLastError() != cudaSuccess) return SACRA_ERR_CUDA;
   }
   return SACRA_OK;
