@@ -1,9 +1,11 @@
 // sacra.cu -- libsacra: C ABI (include/sacra.h) and the CUDA kernels behind it, sm_100a only.
 //
 // Kernels
-//   k_fill_ghosts   periodic halo fill, one block per storage plane and field
-//   k_z4c           derivative stage + algebra + KO + epilogue (RHS store or RK4 substage), one thread
-//                   per active point
+//   k_fill_ghosts   halo fill, periodic or mirror per axis
+//   k_z4c<EPI>      derivative stage + algebra + KO + epilogue (EPI 0: RHS store, 1..4: RK4 substage), one thread
+//                   per active point, persistent CTAs on TMA-staged tiles;
+//                   EPI -1: the constraint monitor on the same machinery
+//   k_con_partial, k_con_final   deterministic volume-normalised L2 norms of the constraints (Eq. 22)
 // There is no CPU path: every entry point enqueues kernels on the caller's stream or returns an error.
 #include <cmath>
 #include <cstdint>

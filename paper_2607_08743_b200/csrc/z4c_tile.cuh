@@ -7,8 +7,11 @@
 // Kreiss-Oliger stencils -- from HBM/L2 into one of NS ring buffers and signals an mbarrier.
 // The ring runs NS-1 fields ahead of the arithmetic and carries on across the tiles of a persistent CTA
 // (the first fields of the next tile are in flight while the last fields of the current one are computed).
-// NS divides 25, so the ring slot of every field is a compile-time constant and every shared-memory load of
-// the stencils has an immediate offset.
+// The ring slot of a field is (tile count * stream length + stream position) % NS: one register per field holds the
+// slot base, every shared-memory load of the stencils has an immediate offset from it.
+// The same machinery serves three more TMA streams: the centre-value tile of all 25 fields (no halo; the values
+// the algebra needs before a field's own box arrives), the ring of RK inputs u_n / acc in emit order (stages
+// 2-4), and -- with a 15-field stream -- the constraint monitor.
 #pragma once
 #include <cstdint>
 #include <type_traits>
