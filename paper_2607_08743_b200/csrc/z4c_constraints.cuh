@@ -25,49 +25,10 @@ __device__ __forceinline__ void constraints_point(const Src& src, double h, Emit
     const double zero[3] = {0.0, 0.0, 0.0};
     make_coef(h, 0.0, zero, pc);
   }
-  // ---- derivatives, field by field ---------------------------------------------------------------------------
-  double dW[3], ddW[6];
-  field_derivs<true, true, false>(src.template field<F_W>(), pc, S);
-  const double W = S.u0;
+  // ---- centre values first (centre tile): metric, its inverse, K, B_ij = At_ij + gt_ij K / 3 -------------------------
+  double g[6], gi[6];
 #pragma unroll
-  for (int k = 0; k < 3; ++k) dW[k] = S.d1[k];
-#pragma unroll
-  for (int n = 0; n < 6; ++n) ddW[n] = S.d2[n];
-
-  double g[6], dg[3][6], ddg[6][6];   // ddg[lm][ij] = d_l d_m gt_ij
-#define GT_FIELD(N)                                                                  \
-  {                                                                                  \
-    field_derivs<true, true, false>(src.template field<F_G + N>(), pc, S);           \
-    g[N] = S.u0;                                                                     \
-    _Pragma("unroll") for (int k = 0; k < 3; ++k) dg[k][N] = S.d1[k];                \
-    _Pragma("unroll") for (int m = 0; m < 6; ++m) ddg[m][N] = S.d2[m];               \
-  }
-  GT_FIELD(0) GT_FIELD(1) GT_FIELD(2) GT_FIELD(3) GT_FIELD(4) GT_FIELD(5)
-#undef GT_FIELD
-
-  double K, dK[3];
-  field_derivs<true, false, false>(src.template field<F_KH>(), pc, S);
-  K = S.u0;
-#pragma unroll
-  for (int k = 0; k < 3; ++k) dK[k] = S.d1[k];
-  field_derivs<true, false, false>(src.template field<F_TH>(), pc, S);
-  K += 2.0 * S.u0;
-#pragma unroll
-  for (int k = 0; k < 3; ++k) dK[k] += 2.0 * S.d1[k];
-
-  double B[6], dB[3][6];              // B_ij = At_ij + gt_ij K / 3 and its gradient
-#define AT_FIELD(N)                                                                  \
-  {                                                                                  \
-    field_derivs<true, false, false>(src.template field<F_A + N>(), pc, S);          \
-    B[N] = S.u0 + g[N] * K / 3.0;                                                    \
-    _Pragma("unroll") for (int k = 0; k < 3; ++k)                                    \
-      dB[k][N] = S.d1[k] + (dg[k][N] * K + g[N] * dK[k]) / 3.0;                      \
-  }
-  AT_FIELD(0) AT_FIELD(1) AT_FIELD(2) AT_FIELD(3) AT_FIELD(4) AT_FIELD(5)
-#undef AT_FIELD
-
-  // ---- inverse conformal metric and its gradient -----------------------------------------------------------------
-  double gi[6];
+  for (int n = 0; n < 6; ++n) g[n] = src.centre(F_G + n);
   {
     const double gxx = g[0], gxy = g[1], gxz = g[2], gyy = g[3], gyz = g[4], gzz = g[5];
     const double det = (gxx * (gyy * gzz - gyz * gyz) - gxy * (gxy * gzz - gyz * gxz)) + gxz * (gxy * gyz - gyy * gxz);
@@ -78,6 +39,65 @@ __device__ __forceinline__ void constraints_point(const Src& src, double h, Emit
     gi[4] = (gxy * gxz - gxx * gyz) / det;
     gi[5] = (gxx * gyy - gxy * gxy) / det;
   }
+  const double K = src.centre(F_KH) + 2.0 * src.centre(F_TH);
+  double B[6];
+#pragma unroll
+  for (int n = 0; n < 6; ++n) B[n] = src.centre(F_A + n) + g[n] * K / 3.0;
+
+  // ---- derivatives, field by field; second derivatives of gt_ij and the gradient of B_ij are folded at once -------
+  double dW[3], ddW[6];
+  field_derivs<true, true, false>(src.template field<F_W>(), pc, S);
+  const double W = S.u0;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) dW[k] = S.d1[k];
+#pragma unroll
+  for (int n = 0; n < 6; ++n) ddW[n] = S.d2[n];
+
+  // second-derivative part of the Ricci scalar of gt:  gt^ij gt^kl ( d_k d_i gt_lj - d_k d_l gt_ij ); the field
+  // gt_ab contributes  m_ab [ (gt^.a)^T D2 (gt^.b) - gt^ab tr(gt^-1 D2) ],  m_ab = 1 (a = b) or 2
+  double dg[3][6], R2 = 0.0;
+#define GT_FIELD(A, Bx)                                                                             \
+  {                                                                                                 \
+    constexpr int N = sym(A, Bx);                                                                   \
+    field_derivs<true, true, false>(src.template field<F_G + N>(), pc, S);                          \
+    _Pragma("unroll") for (int k = 0; k < 3; ++k) dg[k][N] = S.d1[k];                               \
+    double q = 0.0, tr = 0.0;                                                                       \
+    _Pragma("unroll") for (int i = 0; i < 3; ++i)                                                   \
+      _Pragma("unroll") for (int k = 0; k < 3; ++k) {                                               \
+        q = fma(gi[sym(i, A)] * gi[sym(k, Bx)], S.d2[sym(i, k)], q);                                \
+        tr = fma(gi[sym(i, k)], S.d2[sym(i, k)], tr);                                               \
+      }                                                                                             \
+    R2 += (A == Bx ? 1.0 : 2.0) * (q - gi[N] * tr);                                                 \
+  }
+  GT_FIELD(0, 0) GT_FIELD(0, 1) GT_FIELD(0, 2) GT_FIELD(1, 1) GT_FIELD(1, 2) GT_FIELD(2, 2)
+#undef GT_FIELD
+
+  double dK[3];
+  field_derivs<true, false, false>(src.template field<F_KH>(), pc, S);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) dK[k] = S.d1[k];
+  field_derivs<true, false, false>(src.template field<F_TH>(), pc, S);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) dK[k] += 2.0 * S.d1[k];
+
+  // gradient part of the momentum constraint:  gt^ia gt^jb d_j B_ab ; the field B_ab contributes
+  // gt^ia v_b + [a != b] gt^ib v_a  with  v_c = gt^jc d_j B_ab
+  double M[3] = {0.0, 0.0, 0.0};
+#define AT_FIELD(A, Bx)                                                                             \
+  {                                                                                                 \
+    constexpr int N = sym(A, Bx);                                                                   \
+    field_derivs<true, false, false>(src.template field<F_A + N>(), pc, S);                         \
+    double dBn[3];                                                                                  \
+    _Pragma("unroll") for (int k = 0; k < 3; ++k) dBn[k] = S.d1[k] + (dg[k][N] * K + g[N] * dK[k]) / 3.0; \
+    const double va = (gi[sym(0, A)] * dBn[0] + gi[sym(1, A)] * dBn[1]) + gi[sym(2, A)] * dBn[2];   \
+    const double vb = (gi[sym(0, Bx)] * dBn[0] + gi[sym(1, Bx)] * dBn[1]) + gi[sym(2, Bx)] * dBn[2]; \
+    _Pragma("unroll") for (int i = 0; i < 3; ++i)                                                   \
+      M[i] += (A == Bx) ? gi[sym(i, A)] * va : (gi[sym(i, A)] * vb + gi[sym(i, Bx)] * va);          \
+  }
+  AT_FIELD(0, 0) AT_FIELD(0, 1) AT_FIELD(0, 2) AT_FIELD(1, 1) AT_FIELD(1, 2) AT_FIELD(2, 2)
+#undef AT_FIELD
+
+  // ---- gradient of the inverse conformal metric -----------------------------------------------------------------
   double dgi[3][6];                   // d_l gt^ij = - gt^ia gt^jb d_l gt_ab
 #pragma unroll
   for (int l = 0; l < 3; ++l)
@@ -105,26 +125,21 @@ __device__ __forceinline__ void constraints_point(const Src& src, double h, Emit
 #pragma unroll
     for (int n = 0; n < 6; ++n) Gu[k][n] = (gi[sym(k, 0)] * Gl[0][n] + gi[sym(k, 1)] * Gl[1][n]) + gi[sym(k, 2)] * Gl[2][n];
 
-  // ---- Ricci scalar of gt from the derivatives of its Christoffel symbols --------------------------------------
-  double Rt = 0.0;
+  // ---- Ricci scalar of gt: the folded second-derivative part + the first-derivative terms of
+  //      gt^ij ( d_k Gt^k_ij - d_j Gt^k_ik + Gt^k_kl Gt^l_ij - Gt^k_jl Gt^l_ik ) ---------------------------------------
+  double Rt = R2;
 #pragma unroll
   for (int i = 0; i < 3; ++i)
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
       double r = 0.0;
 #pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        // d_k Gt^k_ij = d_k gt^kl Gt_lij + gt^kl d_k Gt_lij ,  d_k Gt_lij = (d_k d_i gt_lj + d_k d_j gt_li - d_k d_l gt_ij)/2
-        // d_j Gt^k_ik = d_j gt^kl Gt_lik + gt^kl d_j Gt_lik
+      for (int k = 0; k < 3; ++k)
 #pragma unroll
         for (int l = 0; l < 3; ++l) {
-          const double dGl_k = 0.5 * ((ddg[sym(k, i)][sym(l, j)] + ddg[sym(k, j)][sym(l, i)]) - ddg[sym(k, l)][sym(i, j)]);
-          const double dGl_j = 0.5 * ((ddg[sym(j, i)][sym(l, k)] + ddg[sym(j, k)][sym(l, i)]) - ddg[sym(j, l)][sym(i, k)]);
-          r += (dgi[k][sym(k, l)] * Gl[l][sym(i, j)] + gi[sym(k, l)] * dGl_k) -
-               (dgi[j][sym(k, l)] * Gl[l][sym(i, k)] + gi[sym(k, l)] * dGl_j);
+          r += dgi[k][sym(k, l)] * Gl[l][sym(i, j)] - dgi[j][sym(k, l)] * Gl[l][sym(i, k)];
           r += Gu[k][sym(k, l)] * Gu[l][sym(i, j)] - Gu[k][sym(j, l)] * Gu[l][sym(i, k)];
         }
-      }
       Rt += gi[sym(i, j)] * r;
     }
   // ---- conformal factor: R = W^2 Rt + 4 W Dt^2 W - 6 |Dt W|^2 -----------------------------------------------------
@@ -158,14 +173,13 @@ __device__ __forceinline__ void constraints_point(const Src& src, double h, Emit
   for (int j = 0; j < 3; ++j) w[j] = dW[j] / W;
 #pragma unroll
   for (int c = 0; c < 3; ++c) wu[c] = (gi[sym(c, 0)] * w[0] + gi[sym(c, 1)] * w[1]) + gi[sym(c, 2)] * w[2];
-  double M[3] = {0.0, 0.0, 0.0};
 #pragma unroll
   for (int j = 0; j < 3; ++j)
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
       for (int b = 0; b < 3; ++b) {
-        double cov = dB[j][sym(a, b)] - 2.0 * w[j] * B[sym(a, b)];
+        double cov = -2.0 * w[j] * B[sym(a, b)];   // the gradient d_j B_ab is already in M
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
           // Gamma^c_ja = Gt^c_ja + C^c_ja ,  C^c_ja = -( delta^c_j w_a + delta^c_a w_j - gt_ja w^c )
