@@ -287,3 +287,18 @@ def test_full_size_config4_sampled_blocks_against_oracle():
             ur = s.active_view(ref, 0, f)[sl, sl, sl]
             assert np.all(np.abs(un - ur) <= p.dt * RTOL * (scale[f] + FLOOR) + np.spacing(np.abs(ur))), \
                 (wl.FIELD_NAMES[f], ctr)
+
+
+def test_rhs_parity_unpadded_pitch():
+    """pitch_x == nx + 6 exactly (nx + 6 a multiple of 8): the tensor maps then address one element more than a row
+    holds (the first cell of the next row), which the boxes never use"""
+    dims = [(10, 10, 10), (42, 6, 6), (26, 7, 9)]
+    ps, total = wl.make_layout(dims, [0.1] * 3, [0.025] * 3, [(0, 0, 0)] * 3)
+    assert all(p.pitch_x == p.nx + 2 * NG for p in ps)
+    w = _smooth_random(wl.Workload("unpadded", ps, dict(wl.DEFAULT_PARAMS), np.zeros(total)), 3)
+    u = w.state.copy()
+    orc.fill_ghosts(ps, u)
+    ref = orc.z4c_rhs(ps, w.params, u)
+    got = gpu_rhs(w, u)
+    assert _untouched_outside_active(w, got)
+    _assert_parity(w, np.nan_to_num(got), ref, "unpadded pitch")
