@@ -159,3 +159,19 @@ def fill_ghosts_bc(ps, mode, u):
     m = (C.c_int32 * 3)(*[int(v) for v in mode])
     lib().orc_fill_ghosts_bc(_patches(ps), len(ps), m, _p(u))
     return u
+
+
+def restrict(parent, child, org, u_parent, u_child):
+    """4th-order Lagrange restriction of the child's active cells onto the covered parent cells, in place on
+    u_parent; org = parent active index of the coarse cell that holds child cells 0, 1 (per axis)."""
+    o = (C.c_int32 * 3)(*[int(v) for v in org])
+    lib().orc_restrict(C.byref(_patches([parent])[0]), C.byref(_patches([child])[0]), o, _p(u_parent), _p(u_child))
+    return u_parent
+
+
+def prolong_ghosts(parent, child, org, u_parent, u_child):
+    """6th-order Lagrange prolongation of the parent onto every ghost cell of the child, in place on u_child"""
+    o = (C.c_int32 * 3)(*[int(v) for v in org])
+    lib().orc_prolong_ghosts(C.byref(_patches([parent])[0]), C.byref(_patches([child])[0]), o, _p(u_parent),
+                             _p(u_child))
+    return u_child

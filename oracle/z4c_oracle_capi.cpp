@@ -11,6 +11,7 @@
 #include <vector>
 #include <omp.h>
 #include "z4c_grid.hpp"
+#include "z4c_amr.hpp"
 
 using namespace z4c_oracle;
 
@@ -92,6 +93,18 @@ void orc_constraints_point(const double* u, const double* d1, const double* d2, 
   static thread_local Derivs<double> D;
   std::memcpy(D.d1, d1, sizeof(D.d1)); std::memcpy(D.d2, d2, sizeof(D.d2));
   constraints_point<double>(u, D, out);
+}
+
+// f-3: spatial inter-level operators (2:1, cell-centred): restriction child -> parent, prolongation of the child's ghosts
+void orc_restrict(const orc_patch* parent, const orc_patch* child, const int32_t* org, double* u_parent,
+                  const double* u_child) {
+  const int o[3] = {org[0], org[1], org[2]};
+  restrict_patch<double>(to_patch(*parent), to_patch(*child), o, u_parent, u_child);
+}
+void orc_prolong_ghosts(const orc_patch* parent, const orc_patch* child, const int32_t* org, const double* u_parent,
+                        double* u_child) {
+  const int o[3] = {org[0], org[1], org[2]};
+  prolong_ghosts<double>(to_patch(*parent), to_patch(*child), o, u_parent, u_child);
 }
 
 // single-point algebra with caller-supplied derivatives (for analytic-derivative pins)
