@@ -131,6 +131,24 @@ int sacra_constraint_norms(const sacra_patch_t* p, int npatch, const double* con
                            void* cuda_stream);
 int64_t sacra_constraint_scratch_doubles(const sacra_patch_t* p, int npatch);
 
+/* Spatial inter-level operators of the box-in-box hierarchy, 2:1 refinement on
+ * cell-centred staggered grids. `parent` and `child` are ONE patch each (HOST pointers; the child has half the
+ * spacing and even nx, ny, nz); org: HOST int32_t[3], the parent ACTIVE-cell index of the coarse cell that holds the
+ * child's active cells 0 and 1 along each axis (its centre lies midway between them). All 25 fields.
+ *   sacra_restrict        every parent cell org + m, 0 <= m < n_child / 2 per axis, is overwritten with the 4-point
+ *                         per axis Lagrange interpolant of the child data at its centre (weights -1 9 9 -1 / 16 on child
+ *                         cells 2m-1 .. 2m+2; the child's ghost cells are read at the patch edges and must be valid).
+ *                         The covered cells must be active cells of the parent.
+ *   sacra_prolong_ghosts  every ghost cell of the child (faces, edges, corners) is overwritten with the 6-point per
+ *                         axis Lagrange interpolant of the parent data at its centre (a quarter of a parent spacing
+ *                         off the parent cell that holds it). Parent cells org + floor(i/2) - 3 .. + 3 are read for
+ *                         child cells i = -3 .. n+2: they must lie in the parent's storage (ghosts included, valid).
+ * Time interpolation and the subcycling driver are not part of the library. */
+int sacra_restrict(const sacra_patch_t* parent, const sacra_patch_t* child, const int32_t* org, double* u_parent,
+                   const double* u_child, void* cuda_stream);
+int sacra_prolong_ghosts(const sacra_patch_t* parent, const sacra_patch_t* child, const int32_t* org,
+                         const double* u_parent, double* u_child, void* cuda_stream);
+
 /* Static description of a status code (never NULL). */
 const char* sacra_strerror(int code);
 

@@ -339,6 +339,106 @@ __global__ void k_con_final(const double* __restrict__ part, int nplanes, double
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Spatial inter-level operators of the box-in-box hierarchy, 2:1 cell-centred
+// staggered grids: along each axis the parent cell org + m holds the child cells 2m and 2m+1. Tensor products of
+// 1-D Lagrange interpolation; the weights are exact dyadic fractions. One thread per target cell and field, sums
+// nested z(y(x)) like the oracle's. HBM/L2-bound and small next to the substage kernel.
+// ---------------------------------------------------------------------------------------------------
+struct LevelPair {
+  DevPatch parent, child;
+  int org[3];
+};
+// restriction: 4 points per axis at the midpoint between child cells 2m and 2m+1 (nodes 2m-1 .. 2m+2)
+__global__ void __launch_bounds__(128) k_restrict(const __grid_constant__ LevelPair L, double* __restrict__ u_parent,
+                                                  const double* __restrict__ u_child) {
+  const DevPatch& pp = L.parent;
+  const DevPatch& pc = L.child;
+  const int hx = pc.nx / 2, hy = pc.ny / 2, hz = pc.nz / 2;
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= hx * hy * hz) return;
+  const int mx = t % hx, my = (t / hx) % hy, mz = t / (hx * hy);
+  const double w[4] = {-1.0 / 16.0, 9.0 / 16.0, 9.0 / 16.0, -1.0 / 16.0};
+  const double* fc = u_child + pc.offset + (long long)blockIdx.y * pc.fstride +
+                     (long long)(2 * mz - 1 + NG) * pc.sz + (long long)(2 * my - 1 + NG) * pc.pitch + (2 * mx - 1 + NG);
+  double az = 0.0;
+#pragma unroll
+  for (int kz = 0; kz < 4; ++kz) {
+    double ay = 0.0;
+#pragma unroll
+    for (int ky = 0; ky < 4; ++ky) {
+      double ax = 0.0;
+#pragma unroll
+      for (int kx = 0; kx < 4; ++kx) ax = ax + w[kx] * fc[(long long)kz * pc.sz + (long long)ky * pc.pitch + kx];
+      ay = ay + w[ky] * ax;
+    }
+    az = az + w[kz] * ay;
+  }
+  u_parent[pp.offset + (long long)blockIdx.y * pp.fstride + (long long)(L.org[2] + mz + NG) * pp.sz +
+           (long long)(L.org[1] + my + NG) * pp.pitch + (L.org[0] + mx + NG)] = az;
+}
+// prolongation of the child's ghost cells: 6 points per axis a quarter of a parent spacing off the parent cell that
+// holds the child cell (to the left for an even child cell, to the right for an odd one: mirrored weights)
+__device__ __forceinline__ void prolong_axis(int i, int org, int& j0, double (&w)[6]) {
+  const double we[6] = {63.0 / 8192.0, -495.0 / 8192.0, 2310.0 / 8192.0, 6930.0 / 8192.0, -693.0 / 8192.0, 77.0 / 8192.0};
+  const int m = i >> 1;                 // floor(i / 2), also for negative i
+  const bool odd = i & 1;
+  j0 = org + m + (odd ? -2 : -3);
+#pragma unroll
+  for (int k = 0; k < 6; ++k) w[k] = odd ? we[5 - k] : we[k];
+}
+__global__ void __launch_bounds__(128) k_prolong_ghosts(const __grid_constant__ LevelPair L, const double* __restrict__ u_parent,
+                                                        double* __restrict__ u_child) {
+  const DevPatch& pp = L.parent;
+  const DevPatch& pc = L.child;
+  const int sx = pc.nx + 2 * NG, sy = pc.ny + 2 * NG;
+  // the ghost shell only: 6 whole z planes, then 6 whole rows of every active plane, then the 6 x-ghosts of every
+  // active row
+  const int nzs = 2 * NG * sx * sy, nys = 2 * NG * sx * pc.nz, nxs = 2 * NG * pc.ny * pc.nz;
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nzs + nys + nxs) return;
+  int I, J, Kk;
+  if (t < nzs) {
+    I = t % sx; J = (t / sx) % sy;
+    const int q = t / (sx * sy);
+    Kk = q < NG ? q : pc.nz + q;
+  } else if (t < nzs + nys) {
+    t -= nzs;
+    I = t % sx;
+    const int q = (t / sx) % (2 * NG);
+    J = q < NG ? q : pc.ny + q;
+    Kk = t / (sx * 2 * NG) + NG;
+  } else {
+    t -= nzs + nys;
+    const int q = t % (2 * NG);
+    I = q < NG ? q : pc.nx + q;
+    J = (t / (2 * NG)) % pc.ny + NG;
+    Kk = t / (2 * NG * pc.ny) + NG;
+  }
+  const int i = I - NG, j = J - NG, k = Kk - NG;
+  int x0, y0, z0;
+  double wx[6], wy[6], wz[6];
+  prolong_axis(i, L.org[0], x0, wx);
+  prolong_axis(j, L.org[1], y0, wy);
+  prolong_axis(k, L.org[2], z0, wz);
+  const double* fp = u_parent + pp.offset + (long long)blockIdx.y * pp.fstride + (long long)(z0 + NG) * pp.sz +
+                     (long long)(y0 + NG) * pp.pitch + (x0 + NG);
+  double az = 0.0;
+#pragma unroll
+  for (int kz = 0; kz < 6; ++kz) {
+    double ay = 0.0;
+#pragma unroll
+    for (int ky = 0; ky < 6; ++ky) {
+      double ax = 0.0;
+#pragma unroll
+      for (int kx = 0; kx < 6; ++kx) ax = ax + wx[kx] * fp[(long long)kz * pp.sz + (long long)ky * pp.pitch + kx];
+      ay = ay + wy[ky] * ax;
+    }
+    az = az + wz[kz] * ay;
+  }
+  u_child[pc.offset + (long long)blockIdx.y * pc.fstride + (long long)Kk * pc.sz + (long long)J * pc.pitch + I] = az;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Host side: validation and launches
 // ---------------------------------------------------------------------------------------------------
 static bool aligned16(const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; }
@@ -606,6 +706,52 @@ int sacra_constraint_norms(const sacra_patch_t* p, int npatch, const double* con
     planes += nb;
   }
   k_con_final<<<1, 4, 0, st>>>(scratch, planes, vol, norms);
+  return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
+}
+
+// f-3: geometry checks shared by the two inter-level calls
+static int check_levels(const sacra_patch_t* parent, const sacra_patch_t* child, const int32_t* org, bool prolong) {
+  if (!parent || !child || !org) return SACRA_ERR_NULL;
+  if (int e = check_patches(parent, 1)) return e;
+  if (int e = check_patches(child, 1)) return e;
+  const int nc[3] = {child->nx, child->ny, child->nz}, np[3] = {parent->nx, parent->ny, parent->nz};
+  for (int a = 0; a < 3; ++a) {
+    if (nc[a] & 1) return SACRA_ERR_BADARG;                                  // a parent cell holds two child cells
+    if (org[a] < 0 || org[a] + nc[a] / 2 > np[a]) return SACRA_ERR_BADARG;   // covered cells are parent active cells
+    // prolongation reads the parent cells org + floor(i/2) - 3 .. + 3 for child cells i = -3 .. n+2: inside the
+    // parent's storage (ghosts included)
+    if (prolong && (org[a] - 2 - 3 < -SACRA_NG || org[a] + (nc[a] + 2) / 2 + 3 > np[a] + SACRA_NG - 1)) return SACRA_ERR_BADARG;
+  }
+  return SACRA_OK;
+}
+static LevelPair level_pair(const sacra_patch_t* parent, const sacra_patch_t* child, const int32_t* org) {
+  LevelPair L;
+  L.parent = to_dev(*parent);
+  L.child = to_dev(*child);
+  for (int a = 0; a < 3; ++a) L.org[a] = org[a];
+  return L;
+}
+
+int sacra_restrict(const sacra_patch_t* parent, const sacra_patch_t* child, const int32_t* org, double* u_parent,
+                   const double* u_child, void* cuda_stream) {
+  if (!u_parent || !u_child) return SACRA_ERR_NULL;
+  if (int e = check_levels(parent, child, org, false)) return e;
+  if (!aligned16(u_parent) || !aligned16(u_child)) return SACRA_ERR_ALIGN;
+  const LevelPair L = level_pair(parent, child, org);
+  const int n = (child->nx / 2) * (child->ny / 2) * (child->nz / 2);
+  k_restrict<<<dim3((n + 127) / 128, NF), 128, 0, static_cast<cudaStream_t>(cuda_stream)>>>(L, u_parent, u_child);
+  return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
+}
+
+int sacra_prolong_ghosts(const sacra_patch_t* parent, const sacra_patch_t* child, const int32_t* org,
+                         const double* u_parent, double* u_child, void* cuda_stream) {
+  if (!u_parent || !u_child) return SACRA_ERR_NULL;
+  if (int e = check_levels(parent, child, org, true)) return e;
+  if (!aligned16(u_parent) || !aligned16(u_child)) return SACRA_ERR_ALIGN;
+  const LevelPair L = level_pair(parent, child, org);
+  const int sx = child->nx + 2 * NG, sy = child->ny + 2 * NG;
+  const int n = 2 * NG * (sx * sy + sx * child->nz + child->ny * child->nz);   // cells of the ghost shell
+  k_prolong_ghosts<<<dim3((n + 127) / 128, NF), 128, 0, static_cast<cudaStream_t>(cuda_stream)>>>(L, u_parent, u_child);
   return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
 }
 

@@ -20,7 +20,7 @@ OK, ERR_NULL, ERR_BADARG, ERR_UNSUPPORTED, ERR_ALIGN, ERR_CUDA = 0, -1, -2, -3, 
 EXPORTS = ("sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4_step",
            "sacra_strerror", "sacra_version",
            "sacra_constraints", "sacra_constraint_norms", "sacra_constraint_scratch_doubles",
-           "sacra_fill_ghosts_bc")
+           "sacra_fill_ghosts_bc", "sacra_restrict", "sacra_prolong_ghosts")
 
 
 class SacraPatch(C.Structure):
@@ -57,7 +57,9 @@ def _load():
     lib.sacra_constraint_scratch_doubles.argtypes = [vp, i32]
     lib.sacra_constraint_scratch_doubles.restype = C.c_int64
     lib.sacra_fill_ghosts_bc.argtypes = [vp, i32, vp, dp, vp]
-    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:10]:
+    lib.sacra_restrict.argtypes = [vp, vp, vp, dp, dp, vp]
+    lib.sacra_prolong_ghosts.argtypes = [vp, vp, vp, dp, dp, vp]
+    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:12]:
         getattr(lib, n).restype = C.c_int
     lib.sacra_strerror.argtypes = [C.c_int]
     lib.sacra_strerror.restype = C.c_char_p
@@ -177,3 +179,19 @@ def fill_ghosts_bc(patches, axis_mode, u, stream=None):
     ps = make_patches(patches) if patches is not None else None
     m = (C.c_int32 * 3)(*[int(v) for v in axis_mode])
     _check(lib.sacra_fill_ghosts_bc(ps, len(ps) if ps is not None else 0, m, _ptr(u), _stream(stream)))
+
+
+def _one(p):
+    return make_patches([p]) if p is not None else None
+
+
+def restrict(parent, child, org, u_parent, u_child, stream=None):
+    """4th-order Lagrange restriction child -> covered parent cells (sacra_restrict)"""
+    o = (C.c_int32 * 3)(*[int(v) for v in org]) if org is not None else None
+    _check(lib.sacra_restrict(_one(parent), _one(child), o, _ptr(u_parent), _ptr(u_child), _stream(stream)))
+
+
+def prolong_ghosts(parent, child, org, u_parent, u_child, stream=None):
+    """6th-order Lagrange prolongation parent -> ghost cells of the child (sacra_prolong_ghosts)"""
+    o = (C.c_int32 * 3)(*[int(v) for v in org]) if org is not None else None
+    _check(lib.sacra_prolong_ghosts(_one(parent), _one(child), o, _ptr(u_parent), _ptr(u_child), _stream(stream)))

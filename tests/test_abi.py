@@ -107,3 +107,19 @@ def test_constraint_monitor_and_bc_fill_argument_checks():
     assert _code(sacra.fill_ghosts_bc, ps, (0, 0, 2), FAKE) == sacra.ERR_BADARG     # unknown mode
     assert _code(sacra.fill_ghosts_bc, ps, (0, 0, 1), None) == sacra.ERR_NULL
     assert _code(sacra.fill_ghosts_bc, ps, (0, 1, 1), FAKE + 8) == sacra.ERR_ALIGN
+
+
+def test_inter_level_argument_checks():
+    pp, _ = wl.make_layout([(16, 16, 16)], [0.2], [0.01], [(0, 0, 0)])
+    pc, _ = wl.make_layout([(8, 8, 8)], [0.1], [0.005], [(0, 0, 0)])
+    odd, _ = wl.make_layout([(7, 8, 8)], [0.1], [0.005], [(0, 0, 0)])
+    ok = (4, 4, 4)
+    assert _code(sacra.restrict, pp[0], pc[0], ok, None, FAKE) == sacra.ERR_NULL
+    assert _code(sacra.restrict, pp[0], pc[0], None, FAKE, FAKE + 64) == sacra.ERR_NULL
+    assert _code(sacra.restrict, pp[0], odd[0], ok, FAKE, FAKE + 64) == sacra.ERR_BADARG        # odd child size
+    assert _code(sacra.restrict, pp[0], pc[0], (13, 4, 4), FAKE, FAKE + 64) == sacra.ERR_BADARG  # past the parent
+    assert _code(sacra.restrict, pp[0], pc[0], (-1, 4, 4), FAKE, FAKE + 64) == sacra.ERR_BADARG
+    assert _code(sacra.restrict, pp[0], pc[0], ok, FAKE + 8, FAKE + 64) == sacra.ERR_ALIGN
+    assert _code(sacra.prolong_ghosts, pp[0], pc[0], (1, 4, 4), FAKE, FAKE + 64) == sacra.ERR_BADARG   # stencil leaves storage
+    assert _code(sacra.prolong_ghosts, pp[0], pc[0], (4, 4, 11), FAKE, FAKE + 64) == sacra.ERR_BADARG
+    assert _code(sacra.prolong_ghosts, pp[0], pc[0], ok, FAKE, None) == sacra.ERR_NULL
