@@ -16,6 +16,9 @@
 #include "z4c_fused.cuh"
 #include "z4c_tile.cuh"
 #include "z4c_constraints.cuh"
+#ifdef SACRA_WS
+#include "z4c_ws.cuh"
+#endif
 
 namespace sacra {
 
@@ -197,7 +200,7 @@ struct TileId {   // a tile of the launch: patch and tile indices
 #endif
 constexpr int SBX = SACRA_SBX, SBY = SACRA_SBY, SBZ = SACRA_SBZ;
 template <class C>
-__device__ __noinline__ TileId locate(const PatchBatch& B, int t) {
+__device__ __forceinline__ TileId locate_inl(const PatchBatch& B, int t) {
   TileId id;
   id.ip = 0;
 #pragma unroll 1
@@ -221,6 +224,10 @@ __device__ __noinline__ TileId locate(const PatchBatch& B, int t) {
   id.bz = sz * SBZ + r / ly;
   return id;
 }
+// out of line in the one-role kernel (its registers are full); a kernel that uses setmaxnreg must not contain calls:
+// ptxas then fails with C7600 "register allocation failed" whatever the targets (found by bisection)
+template <class C>
+__device__ __noinline__ TileId locate(const PatchBatch& B, int t) { return locate_inl<C>(B, t); }
 // map coordinates of the first active cell of a tile: map x coordinate c <-> storage cell c-1 (the maps start
 // one double before storage cell 0, on a 16-byte boundary), active cell i <-> storage cell i + NG
 template <class C>
@@ -294,6 +301,115 @@ __global__ void SACRA_KERNEL_BOUNDS k_z4c(const __grid_constant__ PatchBatch B,
     src.cur = coord<C>(M, id);
   }
 }
+
+#ifdef SACRA_WS
+// ---------------------------------------------------------------------------------------------------
+// Warp-specialised substage kernel (z4c_ws.cuh): warps 0-7 algebra, warps 8-15 derivatives, same tile.
+// ---------------------------------------------------------------------------------------------------
+#ifndef SACRA_WS_REGD
+#define SACRA_WS_REGD 80
+#define SACRA_WS_REGA 176
+#endif
+using WsTile = WsCfg<16, 4, 4, 4, SACRA_WS_REGD, SACRA_WS_REGA>;
+
+template <int EPI>
+__global__ void __launch_bounds__(WsTile::NTHREADS, 1) k_z4c_ws(const __grid_constant__ PatchBatch B,
+                                                                const __grid_constant__ Params P,
+                                                                const __grid_constant__ TileMaps M,
+                                                                double* __restrict__ rhs,
+                                                                const __grid_constant__ RkArgs rk) {
+  using C = WsTile;
+  static_assert(EPI >= 0, "the constraint monitor runs on k_z4c");
+  const int ntiles = B.first_block[B.np];
+  int t = blockIdx.x;
+  if (t >= ntiles) return;
+  const int tid = threadIdx.x;                 // 1-D block of 2 NT threads
+  const int pt = tid % C::NT;                  // point of the tile
+  const int px = pt % C::TX, py = (pt / C::TX) % C::TY, pz = pt / (C::TX * C::TY);
+  TileId* desc = reinterpret_cast<TileId*>(tile_smem + C::BAR_OFF + C::DESC_SLOT);
+  if (tid == 0) {
+    WsBars<C>::init();
+    desc[0] = locate_inl<C>(B, t);
+  }
+  __syncthreads();
+  TileId id = desc[0];
+  const bool more = t + (int)gridDim.x < ntiles;
+
+  if (tid >= C::NT) {
+    // ------------------------------------------------ D warps ------------------------------------------------
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::REG_D));
+    DSide<C> d;
+    d.p = pt;
+    d.lane = tid % 32;
+    d.sc = ((pz + NG) * C::PY + (py + NG)) * C::PX + (px + C::XC);
+    d.ey = C::EY_OFF + (pz * C::TY + py) * C::EX + (px + 2);
+    d.ez = C::EZ_OFF + (pz * (C::TY + 4) + (py + 2)) * C::EX + (px + 2);
+    d.xh = px < 2 ? -2 : (px >= C::TX - 2 ? 2 : 0);
+    d.yh = py < 2 ? -2 : 2;
+    d.iter = 0;
+    d.has_next = more;
+    d.cur = coord<C>(M, id);
+    if (pt == 0) d.prime();
+#pragma unroll 1
+    for (uint32_t iter = 0;; ++iter) {
+      const int tn = t + gridDim.x;
+      d.has_next = tn < ntiles;
+      d.iter = iter;
+      if (pt == 0 && d.has_next) {   // the next tile: for the box prefetch, and for everybody through shared memory
+        const TileId idn = locate_inl<C>(B, tn);
+        desc[(iter + 1) & 1u] = idn;
+        d.nxt = coord<C>(M, idn);
+      }
+      double beta[3];
+      d.shift_at_point(beta);
+      PointCoef pc;
+      make_coef(B.p[id.ip].dx, P.ko_sigma, beta, pc);
+      d.template fields_from<0>(pc);
+      if (!d.has_next) break;
+      t = tn;
+      group_sync<1, C::NT>();          // desc written by the leader at the top of this tile
+      id = desc[(iter + 1) & 1u];
+      d.cur = coord<C>(M, id);
+    }
+  } else {
+    // ------------------------------------------------ A warps ------------------------------------------------
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::REG_A));
+    struct NextTile {
+      const TileMaps* M;
+      const TileId* desc;
+      __device__ __forceinline__ TileCoord next(uint32_t iter) const { return coord<WsTile>(*M, desc[(iter + 1) & 1u]); }
+    };
+    using Src = ASide<C, rk_mode(EPI), NextTile>;
+    Src src;
+    src.geo = NextTile{&M, desc};
+    src.tid = pt;
+    src.lane = tid % 32;
+    src.cen = C::CEN_OFF + pt;
+    src.iter = 0;
+    src.has_next = more;
+    src.cur = coord<C>(M, id);
+    if (pt == 0) src.prime();
+#pragma unroll 1
+    for (uint32_t iter = 0;; ++iter) {
+      const DevPatch& p = B.p[id.ip];
+      const int tn = t + gridDim.x;
+      src.has_next = tn < ntiles;
+      src.iter = iter;
+      const int i = id.bx * C::TX + px, j = id.by * C::TY + py, k = id.bz * C::TZ + pz;
+      const bool active = (i < p.nx) & (j < p.ny) & (k < p.nz);
+      const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
+      Emitter<EPI, Src> emit{src, rhs, rk.u_out, rk.acc, p.offset + c, p.fstride, p.dt, active};
+      src.begin_tile();
+      z4c_point(src, P, p.dx, emit);
+      if (!src.has_next) break;
+      t = tn;
+      id = desc[(iter + 1) & 1u];
+      src.cur = src.nxt;
+    }
+  }
+}
+
+#endif  // SACRA_WS
 
 // ---------------------------------------------------------------------------------------------------
 // Norms of the constraints, Eq. 22: sqrt( sum C^2 dV / sum dV ) over the active cells of all
@@ -541,10 +657,24 @@ static int num_sms() {
   return n;
 }
 
+#ifdef SACRA_WS
+template <int EPI>
+static cudaError_t launch_ws(int grid, cudaStream_t st, const PatchBatch& B, const Params& P, const TileMaps& M,
+                             double* rhs, const RkArgs& rk) {
+  static const cudaError_t attr =
+      cudaFuncSetAttribute(k_z4c_ws<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, WsTile::SMEM_BYTES);
+  if (attr != cudaSuccess) return attr;
+  k_z4c_ws<EPI><<<grid, WsTile::NTHREADS, WsTile::SMEM_BYTES, st>>>(B, P, M, rhs, rk);
+  return cudaGetLastError();
+}
+#endif
+
 template <int EPI>
 static cudaError_t launch_one(int grid, cudaStream_t st, const PatchBatch& B, const Params& P, const TileMaps& M,
                               double* rhs, const RkArgs& rk) {
-
+#ifdef SACRA_WS
+  if constexpr (EPI >= 0) return launch_ws<EPI>(grid, st, B, P, M, rhs, rk);
+#endif
   static const cudaError_t attr =
       cudaFuncSetAttribute(k_z4c<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile::SMEM_BYTES);
   if (attr != cudaSuccess) return attr;
