@@ -14,6 +14,10 @@
 #pragma once
 #include "z4c_tile.cuh"
 
+#ifndef SACRA_WS_NB
+#define SACRA_WS_NB 3   // bundle slots: how far the derivative warps may run ahead of the algebra warps
+#endif
+
 namespace sacra {
 
 __host__ __device__ constexpr bool field_has_d1(int f) { return !(f >= F_A && f < F_A + 6) && !(f >= F_B && f < F_B + 3); }
@@ -30,7 +34,7 @@ struct WsCfg {
   static constexpr int XC = NG + 1;
   static constexpr int PX = TX + 2 * NG + 2, PY = TY + 2 * NG, PZ = TZ + 2 * NG;
   static constexpr int BOX = PX * PY * PZ, BOX_BYTES = BOX * 8, SLOT = (BOX + 15) / 16 * 16;
-  static constexpr int RKD = 5, NB = 2, BW = 12;               // RK ring depth; bundle slots; doubles per bundle
+  static constexpr int RKD = 5, NB = SACRA_WS_NB, BW = 12;     // RK ring depth; bundle slots; doubles per bundle
   // shared-memory map (doubles): ring | mbarriers + tile descriptors | centre tile | RK ring | bundles | e arrays
   static constexpr int BAR_OFF = NS * SLOT;
   static constexpr int CEN_OFF = BAR_OFF + 32;
