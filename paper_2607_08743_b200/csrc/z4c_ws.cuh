@@ -5,12 +5,14 @@
 // warps for the same 16 x 4 x 4 tile: for every point one D thread and one A thread.
 //   D warps (8-15, `setmaxnreg.dec`): own the TMA box ring and the e exchange; for each field, in stream order, they
 //     evaluate the stencils at their point and publish the derivative bundle (u0, D_a, D_ab, advection, KO: 3 to 12
-//     doubles) in a 2-slot bundle ring in shared memory.
+//     doubles) in a bundle ring of SACRA_WS_NB slots in shared memory.
 //   A warps (0-7, `setmaxnreg.inc`): run z4c_point() exactly as before, but src.derivs<F>() only reads the bundle;
 //     they own the centre-value tile, the RK-input ring and the stores.
 // Bundle slots are handed over with full/empty mbarriers (one arrival per warp). Each role keeps its own warps in
 // lockstep with a named barrier (bar.sync 1 / 2 over 256 threads), so the schedulers always have two D and two A warps
 // in different phases to pick from.
+// Status (round 1): runs, bit-identical to the one-role kernel on every GPU test, 8.07 ms per 256^3
+// substage against 7.19 -- an experimental build (-DSACRA_WS), not the default.
 #pragma once
 #include "z4c_tile.cuh"
 
