@@ -16,13 +16,8 @@
 #include "z4c_fused.cuh"
 #include "z4c_tile.cuh"
 #include "z4c_constraints.cuh"
-#ifdef SACRA_WS
-#include "z4c_ws.cuh"
-#endif
 
 namespace sacra {
-
-constexpr int MAXP = 16;   // patch descriptors carried in kernel parameters per launch
 
 struct DevPatch {
   int nx, ny, nz;
@@ -114,19 +109,13 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
 // Fused substage kernel: persistent CTAs, one thread per active point of a TX x TY x TZ tile; the 25 fields
 // are streamed through a TMA ring in shared memory (z4c_tile.cuh).
 // ---------------------------------------------------------------------------------------------------
-#ifndef SACRA_TX   // tile shape (threads per CTA = TX*TY*TZ), ring depth, centre buffers, CTAs per SM: tuning builds
+#ifndef SACRA_TX   // tile shape (threads per CTA = TX*TY*TZ) and ring depth: tuning builds
 #define SACRA_TX 16
 #define SACRA_TY 4
-#define SACRA_TZ 4
-#define SACRA_NS 5
-#define SACRA_CB 2
-#define SACRA_CTAS 1
+#define SACRA_TZ 6
+#define SACRA_NS 4
 #endif
-using Tile = TileCfg<SACRA_TX, SACRA_TY, SACRA_TZ, SACRA_NS, SACRA_CB, SACRA_CTAS>;
-
-struct alignas(64) TileMaps {   // rank-4 (x, y, z, field) tensor maps of every patch of the launch (TileMapSet)
-  CUtensorMap box[MAXP], cen[MAXP], un[MAXP], acc[MAXP];
-};
+using Tile = TileCfg<SACRA_TX, SACRA_TY, SACRA_TZ, SACRA_NS>;
 
 // EPI: 0 = store RHS; 1..4 = RK4 substage (item 11 table)
 struct RkArgs {
@@ -137,7 +126,8 @@ struct RkArgs {
 __host__ __device__ constexpr int rk_mode(int epi) { return epi == 0 ? 0 : (epi == 1 ? 1 : 2); }
 
 // Consumes the finished RHS values. The RK4 inputs never come from global loads: at stage 1 u_n is the stage
-// input itself (centre tile), from stage 2 on u_n and acc arrive through the TMA ring of TileSource.
+// input itself (the centre sample of the field's own box), from stage 2 on u_n and acc arrive through the TMA ring
+// of TileSource.
 // active: out-of-range threads of a ragged tile run the same instruction stream on zero-filled data (they
 // must reach every barrier) and store nothing.
 template <int EPI, class Src>
@@ -149,16 +139,16 @@ struct Emitter {
   long long o, fstride;    // offset of field 0 at this point, field stride
   double dt;
   bool active;
+  // u0: the field's value at the point, which is u_n at stage 1
   template <int F>
-  __device__ __forceinline__ void put(double kk) {
+  __device__ __forceinline__ void put(double kk, double u0) {
     const long long a = o + (long long)F * fstride;
     if (EPI == 0) {
       if (active) __stcs(rhs + a, kk);   // streaming store: written once, not re-read by this launch
       return;
     }
-    double un, ac = 0.0;
-    if (EPI == 1) un = src.centre(F);
-    else src.template rk_inputs<F>(un, ac);
+    double un = u0, ac = 0.0;
+    if (EPI != 1) src.template rk_inputs<F>(un, ac);
     double acc_new, u_new;
     if (EPI == 1) {
       acc_new = kk;
@@ -180,9 +170,6 @@ struct Emitter {
   }
 };
 
-struct TileId {   // a tile of the launch: patch and tile indices
-  int ip, bx, by, bz;
-};
 // Tile order. Tile t of a patch is NOT tile (t % nbx, ...): consecutive tiles fill SUPER-BLOCKS of SBX x SBY x SBZ
 // tiles (64 x 64 x 32 points; 512 tiles = 3.5 waves of the persistent grid), x fastest inside a super-block,
 // super-blocks x fastest across the patch. The tiles in flight at any time then share their halos through L2
@@ -228,23 +215,10 @@ __device__ __forceinline__ TileId locate_inl(const PatchBatch& B, int t) {
 // ptxas then fails with C7600 "register allocation failed" whatever the targets (found by bisection)
 template <class C>
 __device__ __noinline__ TileId locate(const PatchBatch& B, int t) { return locate_inl<C>(B, t); }
-// map coordinates of the first active cell of a tile: map x coordinate c <-> storage cell c-1 (the maps start
-// one double before storage cell 0, on a 16-byte boundary), active cell i <-> storage cell i + NG
-template <class C>
-__device__ __forceinline__ TileCoord coord(const TileMaps& M, const TileId& id) {
-  return TileCoord{{&M.box[id.ip], &M.cen[id.ip], &M.un[id.ip], &M.acc[id.ip]},
-                   id.bx * C::TX + NG + 1, id.by * C::TY + NG, id.bz * C::TZ + NG};
-}
-
 // EPI 0..4: Z4c right-hand side / RK4 substage; EPI == -1: constraint monitor (rhs receives H, M^x, M^y, M^z in
 // fields 0..3)
-#ifdef SACRA_MAXNREG   // tuning builds: cap the registers of the substage kernel (spill sweep)
-#define SACRA_KERNEL_BOUNDS __maxnreg__(SACRA_MAXNREG)
-#else
-#define SACRA_KERNEL_BOUNDS __launch_bounds__(Tile::NT, Tile::CTAS)
-#endif
 template <int EPI>
-__global__ void SACRA_KERNEL_BOUNDS k_z4c(const __grid_constant__ PatchBatch B,
+__global__ void __launch_bounds__(Tile::NT, 1) k_z4c(const __grid_constant__ PatchBatch B,
                                                      const __grid_constant__ Params P,
                                                      const __grid_constant__ TileMaps M,
                                                      double* __restrict__ rhs, const __grid_constant__ RkArgs rk) {
@@ -253,20 +227,29 @@ __global__ void SACRA_KERNEL_BOUNDS k_z4c(const __grid_constant__ PatchBatch B,
   const int ntiles = B.first_block[B.np];
   int t = blockIdx.x;
   if (t >= ntiles) return;
-  // tile descriptors of this and the next tile of the CTA live in the 4 spare slots of the mbarrier area
-  TileId* desc = reinterpret_cast<TileId*>(tile_smem + C::BAR_OFF + 12);
-  static_assert(C::NS + 2 + C::RKD <= 12 && sizeof(TileId) == 16, "descriptor slots");
-  if ((threadIdx.x | threadIdx.y | threadIdx.z) == 0) desc[0] = locate<C>(B, t);
-  __syncthreads();
-  TileId id = desc[0];
+  // tile descriptors of this and the next tile of the CTA live in the 4 spare slots of the mbarrier area, the base
+  // address of the CTA's Tensor Memory in front of them
+  TileId* desc = Src::desc();
+  uint32_t* tm_base = reinterpret_cast<uint32_t*>(tile_smem + C::BAR_OFF + 11);
+  static_assert(C::NS + 1 + C::RKD <= 11 && sizeof(TileId) == 16, "descriptor slots");
   Src src;
+  src.maps = &M;
   src.tid = threadIdx.x + C::TX * (threadIdx.y + C::TY * threadIdx.z);
-  src.cur = coord<C>(M, id);
   if (src.tid == 0) {
-    for (int i = 0; i < C::NS + 2 + C::RKD; ++i) tma::mbar_init(Src::bar(i), 1);
+    desc[0] = locate<C>(B, t);
+    for (int i = 0; i < C::NS + 1 + C::RKD; ++i) tma::mbar_init(Src::bar(i), 1);
     tma::fence_mbar_init();
   }
+  if (src.tid < 32) tmem::alloc_all(tm_base);   // warp 0 owns the allocation (and frees it at the end)
+  tmem::fence_before_sync();
   __syncthreads();
+  tmem::fence_after_sync();
+  TileId id = desc[0];
+  {
+    // the strip of this thread: Tensor Memory lane 32 (warp % 4) + lane, columns of warp / 4
+    const uint32_t warp = (uint32_t)src.tid / 32u;
+    src.tm = *tm_base + (((warp & 3u) * 32u) << 16) + (warp >> 2) * (2u * C::TM_DOUBLES);
+  }
   src.iter = 0;
   src.has_next = t + (int)gridDim.x < ntiles;
   if (src.tid == 0) src.prime();   // loads of the first tile only: nxt is not needed yet
@@ -281,13 +264,8 @@ __global__ void SACRA_KERNEL_BOUNDS k_z4c(const __grid_constant__ PatchBatch B,
     const DevPatch& p = B.p[id.ip];
     const int tn = t + gridDim.x;
     src.has_next = tn < ntiles;
-    if (src.tid == 0 && src.has_next) {   // read by everybody after the barriers of this tile
-      const TileId idn = locate<C>(B, tn);
-      desc[(iter + 1) & 1u] = idn;
-      src.nxt = coord<C>(M, idn);
-    }
+    if (src.tid == 0 && src.has_next) desc[(iter + 1) & 1u] = locate<C>(B, tn);   // read by everybody after the barriers of this tile
     src.iter = iter;
-    src.cen = C::CEN_OFF + (C::CB == 2 ? (iter & 1u) : 0u) * NF * C::NT + src.tid;
     const int i = id.bx * C::TX + threadIdx.x, j = id.by * C::TY + threadIdx.y, k = id.bz * C::TZ + threadIdx.z;
     const bool active = (i < p.nx) & (j < p.ny) & (k < p.nz);
     const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
@@ -298,118 +276,12 @@ __global__ void SACRA_KERNEL_BOUNDS k_z4c(const __grid_constant__ PatchBatch B,
     if (!src.has_next) break;
     t = tn;
     id = desc[(iter + 1) & 1u];   // written by thread 0 at the top of this tile, many barriers ago
-    src.cur = coord<C>(M, id);
   }
+  tmem::fence_before_sync();
+  __syncthreads();                // every thread is done with its strip
+  if (src.tid < 32) tmem::dealloc_all(*tm_base);
 }
 
-#ifdef SACRA_WS
-// ---------------------------------------------------------------------------------------------------
-// Warp-specialised substage kernel (z4c_ws.cuh): warps 0-7 algebra, warps 8-15 derivatives, same tile.
-// ---------------------------------------------------------------------------------------------------
-#ifndef SACRA_WS_REGD
-#define SACRA_WS_REGD 80
-#define SACRA_WS_REGA 176
-#endif
-using WsTile = WsCfg<16, 4, 4, 4, SACRA_WS_REGD, SACRA_WS_REGA>;
-
-template <int EPI>
-__global__ void __launch_bounds__(WsTile::NTHREADS, 1) k_z4c_ws(const __grid_constant__ PatchBatch B,
-                                                                const __grid_constant__ Params P,
-                                                                const __grid_constant__ TileMaps M,
-                                                                double* __restrict__ rhs,
-                                                                const __grid_constant__ RkArgs rk) {
-  using C = WsTile;
-  static_assert(EPI >= 0, "the constraint monitor runs on k_z4c");
-  const int ntiles = B.first_block[B.np];
-  int t = blockIdx.x;
-  if (t >= ntiles) return;
-  const int tid = threadIdx.x;                 // 1-D block of 2 NT threads
-  const int pt = tid % C::NT;                  // point of the tile
-  const int px = pt % C::TX, py = (pt / C::TX) % C::TY, pz = pt / (C::TX * C::TY);
-  TileId* desc = reinterpret_cast<TileId*>(tile_smem + C::BAR_OFF + C::DESC_SLOT);
-  if (tid == 0) {
-    WsBars<C>::init();
-    desc[0] = locate_inl<C>(B, t);
-  }
-  __syncthreads();
-  TileId id = desc[0];
-  const bool more = t + (int)gridDim.x < ntiles;
-
-  if (tid >= C::NT) {
-    // ------------------------------------------------ D warps ------------------------------------------------
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::REG_D));
-    DSide<C> d;
-    d.p = pt;
-    d.lane = tid % 32;
-    d.sc = ((pz + NG) * C::PY + (py + NG)) * C::PX + (px + C::XC);
-    d.ey = C::EY_OFF + (pz * C::TY + py) * C::EX + (px + 2);
-    d.ez = C::EZ_OFF + (pz * (C::TY + 4) + (py + 2)) * C::EX + (px + 2);
-    d.xh = px < 2 ? -2 : (px >= C::TX - 2 ? 2 : 0);
-    d.yh = py < 2 ? -2 : 2;
-    d.iter = 0;
-    d.has_next = more;
-    d.cur = coord<C>(M, id);
-    if (pt == 0) d.prime();
-#pragma unroll 1
-    for (uint32_t iter = 0;; ++iter) {
-      const int tn = t + gridDim.x;
-      d.has_next = tn < ntiles;
-      d.iter = iter;
-      if (pt == 0 && d.has_next) {   // the next tile: for the box prefetch, and for everybody through shared memory
-        const TileId idn = locate_inl<C>(B, tn);
-        desc[(iter + 1) & 1u] = idn;
-        d.nxt = coord<C>(M, idn);
-      }
-      double beta[3];
-      d.shift_at_point(beta);
-      PointCoef pc;
-      make_coef(B.p[id.ip].dx, P.ko_sigma, beta, pc);
-      d.template fields_from<0>(pc);
-      if (!d.has_next) break;
-      t = tn;
-      group_sync<1, C::NT>();          // desc written by the leader at the top of this tile
-      id = desc[(iter + 1) & 1u];
-      d.cur = coord<C>(M, id);
-    }
-  } else {
-    // ------------------------------------------------ A warps ------------------------------------------------
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::REG_A));
-    struct NextTile {
-      const TileMaps* M;
-      const TileId* desc;
-      __device__ __forceinline__ TileCoord next(uint32_t iter) const { return coord<WsTile>(*M, desc[(iter + 1) & 1u]); }
-    };
-    using Src = ASide<C, rk_mode(EPI), NextTile>;
-    Src src;
-    src.geo = NextTile{&M, desc};
-    src.tid = pt;
-    src.lane = tid % 32;
-    src.cen = C::CEN_OFF + pt;
-    src.iter = 0;
-    src.has_next = more;
-    src.cur = coord<C>(M, id);
-    if (pt == 0) src.prime();
-#pragma unroll 1
-    for (uint32_t iter = 0;; ++iter) {
-      const DevPatch& p = B.p[id.ip];
-      const int tn = t + gridDim.x;
-      src.has_next = tn < ntiles;
-      src.iter = iter;
-      const int i = id.bx * C::TX + px, j = id.by * C::TY + py, k = id.bz * C::TZ + pz;
-      const bool active = (i < p.nx) & (j < p.ny) & (k < p.nz);
-      const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
-      Emitter<EPI, Src> emit{src, rhs, rk.u_out, rk.acc, p.offset + c, p.fstride, p.dt, active};
-      src.begin_tile();
-      z4c_point(src, P, p.dx, emit);
-      if (!src.has_next) break;
-      t = tn;
-      id = desc[(iter + 1) & 1u];
-      src.cur = src.nxt;
-    }
-  }
-}
-
-#endif  // SACRA_WS
 
 // ---------------------------------------------------------------------------------------------------
 // Norms of the constraints, Eq. 22: sqrt( sum C^2 dV / sum dV ) over the active cells of all
@@ -657,24 +529,10 @@ static int num_sms() {
   return n;
 }
 
-#ifdef SACRA_WS
-template <int EPI>
-static cudaError_t launch_ws(int grid, cudaStream_t st, const PatchBatch& B, const Params& P, const TileMaps& M,
-                             double* rhs, const RkArgs& rk) {
-  static const cudaError_t attr =
-      cudaFuncSetAttribute(k_z4c_ws<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, WsTile::SMEM_BYTES);
-  if (attr != cudaSuccess) return attr;
-  k_z4c_ws<EPI><<<grid, WsTile::NTHREADS, WsTile::SMEM_BYTES, st>>>(B, P, M, rhs, rk);
-  return cudaGetLastError();
-}
-#endif
 
 template <int EPI>
 static cudaError_t launch_one(int grid, cudaStream_t st, const PatchBatch& B, const Params& P, const TileMaps& M,
                               double* rhs, const RkArgs& rk) {
-#ifdef SACRA_WS
-  if constexpr (EPI >= 0) return launch_ws<EPI>(grid, st, B, P, M, rhs, rk);
-#endif
   static const cudaError_t attr =
       cudaFuncSetAttribute(k_z4c<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile::SMEM_BYTES);
   if (attr != cudaSuccess) return attr;
@@ -707,7 +565,7 @@ static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* 
       }
     }
     B.first_block[B.np] = nb;
-    const int grid = nb < sms * Tile::CTAS ? nb : sms * Tile::CTAS;   // persistent CTAs, tiles dealt round-robin
+    const int grid = nb < sms ? nb : sms;   // persistent CTAs (one per SM: the kernel owns the SM's Tensor Memory)
     cudaError_t err;
     switch (epi) {
       case -1: err = launch_one<-1>(grid, st, B, P, M, rhs, rk); break;

@@ -14,6 +14,7 @@
 // instruction stream.
 #pragma once
 #include "z4c_stencil.cuh"
+#include "z4c_tile.cuh"
 
 namespace sacra {
 
@@ -25,10 +26,19 @@ __device__ __forceinline__ void constraints_point(const Src& src, double h, Emit
     const double zero[3] = {0.0, 0.0, 0.0};
     make_coef(h, 0.0, zero, pc);
   }
-  // ---- centre values first (centre tile): metric, its inverse, K, B_ij = At_ij + gt_ij K / 3 -------------------------
-  double g[6], gi[6];
-#pragma unroll
-  for (int n = 0; n < 6; ++n) g[n] = src.centre(F_G + n);
+  // ---- centre values first (Tensor Memory strip): metric, its inverse, K, B_ij = At_ij + gt_ij K / 3 ----------------
+  double g[6], gi[6], A[6], Kh, Th;
+  {
+    using namespace tmem;
+    Pack4 p0, p8, p12, p16;
+    Pack2 p4, p20;
+    ld4(src.strip(0), p0); ld2(src.strip(4), p4); ld4(src.strip(8), p8); ld4(src.strip(12), p12);
+    ld4(src.strip(16), p16); ld2(src.strip(20), p20);
+    wait_ld(p0, p4, p8, p12, p16, p20);
+    g[0] = p0.get(0); g[1] = p0.get(1); g[2] = p0.get(2); g[3] = p0.get(3); g[4] = p4.get(0); g[5] = p4.get(1);
+    Kh = p8.get(3); Th = p12.get(3);
+    A[0] = p16.get(0); A[1] = p16.get(1); A[2] = p16.get(2); A[3] = p16.get(3); A[4] = p20.get(0); A[5] = p20.get(1);
+  }
   {
     const double gxx = g[0], gxy = g[1], gxz = g[2], gyy = g[3], gyz = g[4], gzz = g[5];
     const double det = (gxx * (gyy * gzz - gyz * gyz) - gxy * (gxy * gzz - gyz * gxz)) + gxz * (gxy * gyz - gyy * gxz);
@@ -39,10 +49,10 @@ __device__ __forceinline__ void constraints_point(const Src& src, double h, Emit
     gi[4] = (gxy * gxz - gxx * gyz) / det;
     gi[5] = (gxx * gyy - gxy * gxy) / det;
   }
-  const double K = src.centre(F_KH) + 2.0 * src.centre(F_TH);
+  const double K = Kh + 2.0 * Th;
   double B[6];
 #pragma unroll
-  for (int n = 0; n < 6; ++n) B[n] = src.centre(F_A + n) + g[n] * K / 3.0;
+  for (int n = 0; n < 6; ++n) B[n] = A[n] + g[n] * K / 3.0;
 
   // ---- derivatives, field by field; second derivatives of gt_ij and the gradient of B_ij are folded at once -------
   double dW[3], ddW[6];
@@ -165,7 +175,7 @@ __device__ __forceinline__ void constraints_point(const Src& src, double h, Emit
   for (int i = 0; i < 3; ++i)
 #pragma unroll
     for (int j = 0; j < 3; ++j) BB += Bu[i][j] * Bu[j][i];
-  emit.template put<0>(R + K * K - BB);
+  emit.template put<0>(R + K * K - BB, 0.0);
 
   // ---- momentum constraint ------------------------------------------------------------------------------------------
   double w[3], wu[3];                 // w_j = d_j W / W, w^c = gt^cd w_d
@@ -192,9 +202,9 @@ __device__ __forceinline__ void constraints_point(const Src& src, double h, Emit
       }
 #pragma unroll
   for (int i = 0; i < 3; ++i) M[i] -= (gi[sym(i, 0)] * dK[0] + gi[sym(i, 1)] * dK[1]) + gi[sym(i, 2)] * dK[2];
-  emit.template put<1>(W * W * M[0]);
-  emit.template put<2>(W * W * M[1]);
-  emit.template put<3>(W * W * M[2]);
+  emit.template put<1>(W * W * M[0], 0.0);
+  emit.template put<2>(W * W * M[1], 0.0);
+  emit.template put<3>(W * W * M[2], 0.0);
 }
 
 }  // namespace sacra

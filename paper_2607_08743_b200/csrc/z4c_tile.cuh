@@ -10,14 +10,16 @@
 // The ring slot of a field is (tile count * stream length + stream position) % NS: one register per field holds the
 // slot base, every shared-memory load of the stencils has an immediate offset from it.
 // The same machinery serves three more TMA streams: the centre-value tile of all 25 fields (no halo; the values
-// the algebra needs before a field's own box arrives), the ring of RK inputs u_n / acc in emit order (stages
-// 2-4), and -- with a 15-field stream -- the constraint monitor.
+// the algebra needs before a field's own box arrives; every thread copies its 25 values into its Tensor Memory
+// strip at the start of a tile, z4c_tmem.cuh, which frees the buffer for the next tile's values), the ring of RK
+// inputs u_n / acc in emit order (stages 2-4), and -- with a 15-field stream -- the constraint monitor.
 #pragma once
 #include <cstdint>
 #include <type_traits>
 #include <cuda.h>   // CUtensorMap (types only; the encoder is fetched through cudaGetDriverEntryPoint)
 
 #include "z4c_stencil.cuh"
+#include "z4c_tmem.cuh"
 
 namespace sacra {
 
@@ -111,12 +113,40 @@ __device__ __forceinline__ void load_box(void* dst, const CUtensorMap* map, uint
 }
 }  // namespace tma
 
-template <int TX_, int TY_, int TZ_, int NS_, int CB_, int CTAS_>
+// ---- the Tensor Memory strip of a thread (z4c_tmem.cuh), in doubles ------------------------------------------------
+// centre values of the 25 fields, grouped the way z4c_point() pulls them (aligned groups of 4 / 2 / 1 doubles):
+//   0-5 gt_ij | 6 alpha | 7 W | 8-10 beta^i | 11 K-hat | 12-14 B^i | 15 Theta | 16-21 At_ij | 22-24 Gt^i
+// then the parked tensors of the algebra.
+__host__ __device__ constexpr int cen_slot(int f) {
+  return (f >= F_G && f < F_G + 6) ? f - F_G
+       : f == F_ALP ? 6 : f == F_W ? 7
+       : (f >= F_BET && f < F_BET + 3) ? 8 + (f - F_BET)
+       : f == F_KH ? 11
+       : (f >= F_B && f < F_B + 3) ? 12 + (f - F_B)
+       : f == F_TH ? 15
+       : (f >= F_A && f < F_A + 6) ? 16 + (f - F_A)
+       : 22 + (f - F_GAM);
+}
+__host__ __device__ constexpr int cen_field(int slot) {
+  for (int f = 0; f < NF; ++f)
+    if (cen_slot(f) == slot) return f;
+  return -1;
+}
+constexpr int PK_DB = 28;    // d_k beta^i, 3 groups k of 4 doubles (i = 0..2, pad)
+constexpr int PK_DG = 40;    // d_k gt_n,   6 groups n of 4 doubles (k = 0..2, pad); later Gt^k_n in the same place
+constexpr int PK_GU = PK_DG;
+constexpr int PK_AUU = 64;   // At^ij,      3 groups i of 4 doubles (j = 0..2, pad)
+constexpr int PK_AG = 76;    // advection and KO of Gt^k, 3 groups k of 2 doubles
+constexpr int PK_END = 82;
+
+template <int TX_, int TY_, int TZ_, int NS_>
 struct TileCfg {
   static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NS = NS_;
-  static constexpr int CB = CB_;       // centre-value buffers: 2 = the next tile's values load during this tile
-  static constexpr int CTAS = CTAS_;   // CTAs per SM the launch is sized for
   static constexpr int NT = TX * TY * TZ;                      // threads = points per tile
+  // Tensor Memory: 512 columns shared by the warps of a lane quarter (warps w, w + 4, ...): doubles per thread
+  static constexpr int TM_WARPS = (NT / 32 + 3) / 4;
+  static constexpr int TM_DOUBLES = (512 / TM_WARPS) / 2 / 2 * 2;
+  static_assert(NT % 128 == 0 && PK_END <= TM_DOUBLES, "Tensor Memory strip of a thread");
   // box extents. x: the box must start on a 16-byte boundary of global memory (TMA rule for the innermost
   // coordinate, found by probing: an odd FP64 start coordinate raises "illegal instruction"); storage cell
   // bx*TX of a row sits at an odd double (sacra.h), so the box starts one cell earlier and is one cell wider
@@ -127,25 +157,24 @@ struct TileCfg {
   static constexpr int BOX_BYTES = BOX * 8;
   static constexpr int SLOT = (BOX + 15) / 16 * 16;            // doubles per ring slot (128-byte multiple)
   // shared-memory map (in doubles):
-  //   ring | mbarriers | centre tiles (CB x NF x NT) | RK ring (RKD x {u_n, acc} x NT) | E_y | E_z
+  //   ring | mbarriers | centre tile (NF x NT) | RK ring (RKD x {u_n, acc} x NT) | E_y | E_z
   static constexpr int RKD = 5;                                // depth of the RK-input ring (divides NF)
-  static constexpr int BAR_OFF = NS * SLOT;                    // NS box + 2 centre + RKD rk mbarriers (16 reserved)
-  static constexpr int CEN_OFF = BAR_OFF + 16;                 // unpadded tiles of all NF fields, CB buffers
+  static constexpr int BAR_OFF = NS * SLOT;                    // NS box + 1 centre + RKD rk mbarriers (16 reserved)
+  static constexpr int CEN_OFF = BAR_OFF + 16;                 // unpadded tiles of all NF fields
   static constexpr int CEN_BYTES = NF * NT * 8;
-  static constexpr int RK_OFF = CEN_OFF + CB * NF * NT;         // slot r: u_n tile at RK_OFF + 2 r NT, acc tile + NT
+  static constexpr int RK_OFF = CEN_OFF + NF * NT;             // slot r: u_n tile at RK_OFF + 2 r NT, acc tile + NT
   static constexpr int EX = TX + 4;                            // x extent of the e arrays (x halo of 2)
   static constexpr int EY_OFF = RK_OFF + RKD * 2 * NT;         // e_y on  TZ x TY x (TX+4)
   static constexpr int EZ_OFF = EY_OFF + TZ * TY * EX;         // e_z on  TZ x (TY+4) x (TX+4)
   static constexpr int ESZ = TZ * TY * EX + TZ * (TY + 4) * EX;   // one set of e arrays
   // with room for a second set of e arrays, fields with mixed derivatives need one block barrier instead of two
   // (MERGE: the ring refill waits for the barrier of the e exchange; the sets alternate)
-  static constexpr bool MERGE = (EY_OFF + 2 * ESZ) * 8 * CTAS + 1024 * CTAS <= 233472;
+  static constexpr bool MERGE = (EY_OFF + 2 * ESZ) * 8 + 1024 <= 233472;
   static constexpr int SMEM_BYTES = (EY_OFF + (MERGE ? 2 : 1) * ESZ) * 8;
-  static_assert(SMEM_BYTES * CTAS + 1024 * CTAS <= 233472, "shared memory of the CTAs of one SM");
-  static_assert(NF % RKD == 0 && NS + 2 + RKD <= 16, "mbarrier area / RK ring depth");
+  static_assert(SMEM_BYTES + 1024 <= 233472, "shared memory of one SM");
+  static_assert(NF % RKD == 0 && NS + 2 + RKD <= 12, "mbarrier area / RK ring depth");
   static_assert(TY == 4 && TX >= 4, "e exchange: one y-halo row of e_z per thread row, x-halo columns by the edge lanes");
   static_assert((NT * 8) % 128 == 0 && SLOT % 16 == 0, "TMA destinations are 128-byte aligned");
-  static_assert(NS <= 8, "mbarrier area");
   static_assert(NS >= 2 && NS <= 5, "ring depth");
   static_assert((PX * 8) % 16 == 0, "TMA: the innermost box extent must be a multiple of 16 bytes");
 };
@@ -221,15 +250,15 @@ __host__ __device__ constexpr int emits_before(int s) {
   return n;
 }
 
-struct TileMapSet {   // tensor maps of one patch (all rank 4: x, y, z, field)
-  const CUtensorMap* box;   // stage input u_in, box  PX x PY x PZ x 1   (stencil tiles)
-  const CUtensorMap* cen;   // stage input u_in, box  TX x TY x TZ x NF  (centre values of every field)
-  const CUtensorMap* un;    // u_n,              box  TX x TY x TZ x 1   (stages 2-4)
-  const CUtensorMap* acc;   // acc,              box  TX x TY x TZ x 1   (stages 2-4)
+constexpr int MAXP = 16;   // patch descriptors carried in kernel parameters per launch
+struct alignas(64) TileMaps {   // rank-4 (x, y, z, field) tensor maps of every patch of the launch
+  CUtensorMap box[MAXP];   // stage input u_in, box  PX x PY x PZ x 1   (stencil tiles)
+  CUtensorMap cen[MAXP];   // stage input u_in, box  TX x TY x TZ x NF  (centre values of every field)
+  CUtensorMap un[MAXP];    // u_n,              box  TX x TY x TZ x 1   (stages 2-4)
+  CUtensorMap acc[MAXP];   // acc,              box  TX x TY x TZ x 1   (stages 2-4)
 };
-struct TileCoord {   // a tile: the maps of its patch and the map coordinates of its first active cell
-  TileMapSet m;
-  int x, y, z;       // coordinate of active cell (i0, j0, k0): storage (i0+3, j0+3, k0+3) = map (i0+4, j0+3, k0+3)
+struct TileId {   // a tile of the launch: patch and tile indices
+  int ip, bx, by, bz;
 };
 
 // Source for z4c_point(): field<F>() advances the TMA ring to field F and returns its tile loader;
@@ -239,19 +268,29 @@ template <class C, int RK, class Stream = Z4cStream>
 struct TileSource {
   int tid;                 // linear thread index = point of the tile
   int sc;                  // shared memory: index of this thread's centre in ring slot 0
-  int cen;                 // shared memory: this thread's entry of field 0 in the centre tile of this tile
+  uint32_t tm;             // Tensor Memory: address of double 0 of this thread's strip (a double = 2 columns)
   int ey, ez;              // shared memory: this thread's entries of the e arrays
   int xh, yh;              // halo duties of the e exchange (TileLoader)
-  TileCoord cur, nxt;      // this tile and the CTA's next tile
+  const TileMaps* maps;    // kernel parameter (constant bank): costs no register
   bool has_next;
   uint32_t iter;           // tiles done by this CTA (ring phases)
 
   __device__ __forceinline__ static uint64_t* bar(int i) { return reinterpret_cast<uint64_t*>(tile_smem + C::BAR_OFF) + i; }
   __device__ __forceinline__ static uint64_t* full(int slot) { return bar(slot); }            // box landed
-  __device__ __forceinline__ static uint64_t* cen_full(int b) { return bar(C::NS + b); }      // centre tile landed
-  __device__ __forceinline__ static uint64_t* rk_full(int r) { return bar(C::NS + 2 + r); }   // RK inputs landed
+  __device__ __forceinline__ static uint64_t* cen_full() { return bar(C::NS); }               // centre tile landed
+  __device__ __forceinline__ static uint64_t* rk_full(int r) { return bar(C::NS + 1 + r); }   // RK inputs landed
 
-  __device__ __forceinline__ double centre(int f) const { return tile_smem[cen + f * C::NT]; }
+  // descriptors of this tile and of the CTA's next tile: two slots in shared memory, written by the leader (only the
+  // leader needs tile coordinates: they stay out of the registers of everybody else)
+  __device__ __forceinline__ static TileId* desc() { return reinterpret_cast<TileId*>(tile_smem + C::BAR_OFF + 12); }
+  __device__ __forceinline__ TileId tile(bool next) const { return desc()[(iter + (next ? 1u : 0u)) & 1u]; }
+  // map coordinates of the first active cell of a tile: map x coordinate c <-> storage cell c-1 (the maps start one
+  // double before storage cell 0, on a 16-byte boundary), active cell i <-> storage cell i + NG
+  __device__ __forceinline__ static int cx(const TileId& t) { return t.bx * C::TX + NG + 1; }
+  __device__ __forceinline__ static int cy(const TileId& t) { return t.by * C::TY + NG; }
+  __device__ __forceinline__ static int cz(const TileId& t) { return t.bz * C::TZ + NG; }
+
+  __device__ __forceinline__ uint32_t strip(int d) const { return tm + 2u * (uint32_t)d; }    // double d of the strip
 
   // ring slot and use count of stream position s of tile `it` of this CTA: global sequence number it*NF + s
   __device__ __forceinline__ static uint32_t ring_slot(uint32_t it, int s) { return (it * Stream::N + s) % C::NS; }
@@ -262,24 +301,26 @@ struct TileSource {
   __device__ __forceinline__ void issue() const {
     if (S >= Stream::N && !has_next) return;
     constexpr int f = Stream::field(S % Stream::N);
-    const TileCoord& t = S < Stream::N ? cur : nxt;
+    const TileId t = tile(S >= Stream::N);
     const uint32_t slot = ring_slot(iter, S);
     tma::mbar_expect_tx(full(slot), C::BOX_BYTES);
     // the box starts XC cells before the first active cell in x (an even map coordinate) and NG in y, z
-    tma::load_box(tile_smem + slot * C::SLOT, t.m.box, full(slot), t.x - C::XC, t.y - NG, t.z - NG, f,
+    tma::load_box(tile_smem + slot * C::SLOT, &maps->box[t.ip], full(slot), cx(t) - C::XC, cy(t) - NG, cz(t) - NG, f,
                   tma::SACRA_BOX_POLICY);
   }
-  __device__ __forceinline__ static void issue_centre(const TileCoord& t, uint32_t buf) {
-    tma::mbar_expect_tx(cen_full(buf), C::CEN_BYTES);
-    tma::load_box(tile_smem + C::CEN_OFF + buf * NF * C::NT, t.m.cen, cen_full(buf), t.x, t.y, t.z, 0,
-                  tma::SACRA_CEN_POLICY);
+  __device__ __forceinline__ void issue_centre(bool next) const {
+    const TileId t = tile(next);
+    tma::mbar_expect_tx(cen_full(), C::CEN_BYTES);
+    tma::load_box(tile_smem + C::CEN_OFF, &maps->cen[t.ip], cen_full(), cx(t), cy(t), cz(t), 0, tma::SACRA_CEN_POLICY);
   }
   template <int E>
-  __device__ __forceinline__ static void issue_rk(const TileCoord& t) {
+  __device__ __forceinline__ void issue_rk(bool next) const {
     constexpr int r = E % C::RKD, f = emit_field(E);
+    const TileId t = tile(next);
     tma::mbar_expect_tx(rk_full(r), 2 * C::NT * 8);
-    tma::load_box(tile_smem + C::RK_OFF + 2 * r * C::NT, t.m.un, rk_full(r), t.x, t.y, t.z, f, tma::L2_EVICT_FIRST);
-    tma::load_box(tile_smem + C::RK_OFF + (2 * r + 1) * C::NT, t.m.acc, rk_full(r), t.x, t.y, t.z, f,
+    tma::load_box(tile_smem + C::RK_OFF + 2 * r * C::NT, &maps->un[t.ip], rk_full(r), cx(t), cy(t), cz(t), f,
+                  tma::L2_EVICT_FIRST);
+    tma::load_box(tile_smem + C::RK_OFF + (2 * r + 1) * C::NT, &maps->acc[t.ip], rk_full(r), cx(t), cy(t), cz(t), f,
                   tma::L2_EVICT_FIRST);
   }
   // RK inputs of emits (LO, HI]: emit indices >= NF belong to the next tile
@@ -287,14 +328,14 @@ struct TileSource {
   __device__ __forceinline__ void issue_rk_range() const {
     if constexpr (LO < HI) {
       constexpr int e = LO + 1;
-      if constexpr (e < NF) issue_rk<e>(cur);
-      else if (has_next) issue_rk<e - NF>(nxt);
+      if constexpr (e < NF) issue_rk<e>(false);
+      else if (has_next) issue_rk<e - NF>(true);
       issue_rk_range<LO + 1, HI>();
     }
   }
   // what the leader has in flight before the first field<>() call of a CTA
   __device__ __forceinline__ void prime() const {
-    issue_centre(cur, 0);
+    issue_centre(false);
     issue<0>();
     if constexpr (C::NS > 2) issue<1>();
     if constexpr (C::NS > 3) issue<2>();
@@ -302,18 +343,18 @@ struct TileSource {
     if constexpr (RK == 2) issue_rk_range<-1, C::RKD - 2>();
   }
 
-  // start of a tile: every thread is done with the previous tile. CB = 2: its centre buffer takes the next
-  // tile's values while this tile runs. CB = 1: this tile's values can only be requested now (a second CTA on the
-  // SM covers the wait). Then wait for this tile's centre values.
+  // start of a tile: every thread copies its centre values from the shared-memory tile into its Tensor Memory strip
+  // (slot order of cen_slot()). After the first block barrier of the tile the buffer is free and the leader requests
+  // the next tile's values (refill<0>()).
   __device__ __forceinline__ void begin_tile() const {
-    __syncthreads();
-    if constexpr (C::CB == 2) {
-      if (tid == 0 && has_next) issue_centre(nxt, (iter + 1) & 1u);
-      tma::mbar_wait(cen_full(iter & 1u), (iter >> 1) & 1u);
-    } else {
-      if (tid == 0 && iter > 0) issue_centre(cur, 0);
-      tma::mbar_wait(cen_full(0), iter & 1u);
-    }
+    tma::mbar_wait(cen_full(), iter & 1u);
+    const double* c = tile_smem + C::CEN_OFF + tid;
+#pragma unroll
+    for (int q = 0; q < 24; q += 4)
+      tmem::st4(strip(q), c[cen_field(q) * C::NT], c[cen_field(q + 1) * C::NT], c[cen_field(q + 2) * C::NT],
+                c[cen_field(q + 3) * C::NT]);
+    tmem::st1(strip(24), c[cen_field(24) * C::NT]);
+    tmem::wait_st();
   }
 
   // number of fields with mixed derivatives before stream position s (the e-array sets alternate between them)
@@ -331,6 +372,9 @@ struct TileSource {
   // leader: every thread is done with the slot of field s-1 and with every RK slot read so far -- refill them
   template <int s>
   __device__ __forceinline__ void refill() const {
+    if constexpr (s == 0) {
+      if (has_next) issue_centre(true);
+    }
     issue<s + C::NS - 1>();
     if constexpr (RK == 2) {
       // emit e may be loaded once emit e - RKD is done: through emits_before(s) + RKD - 1
