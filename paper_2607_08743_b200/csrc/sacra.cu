@@ -211,75 +211,73 @@ __device__ __forceinline__ TileId locate_inl(const PatchBatch& B, int t) {
   id.bz = sz * SBZ + r / ly;
   return id;
 }
-// out of line in the one-role kernel (its registers are full); a kernel that uses setmaxnreg must not contain calls:
-// ptxas then fails with C7600 "register allocation failed" whatever the targets (found by bisection)
-template <class C>
-__device__ __noinline__ TileId locate(const PatchBatch& B, int t) { return locate_inl<C>(B, t); }
 // EPI 0..4: Z4c right-hand side / RK4 substage; EPI == -1: constraint monitor (rhs receives H, M^x, M^y, M^z in
 // fields 0..3)
 template <int EPI>
-__global__ void __launch_bounds__(Tile::NT, 1) k_z4c(const __grid_constant__ PatchBatch B,
-                                                     const __grid_constant__ Params P,
-                                                     const __grid_constant__ TileMaps M,
-                                                     double* __restrict__ rhs, const __grid_constant__ RkArgs rk) {
+__global__ void __launch_bounds__(Tile::NTH, 1) k_z4c(const __grid_constant__ PatchBatch B,
+                                                      const __grid_constant__ Params P,
+                                                      const __grid_constant__ TileMaps M,
+                                                      double* __restrict__ rhs, const __grid_constant__ RkArgs rk) {
   using C = Tile;
   using Src = TileSource<C, rk_mode(EPI < 0 ? 0 : EPI), std::conditional_t<EPI < 0, ConStream, Z4cStream>>;
   const int ntiles = B.first_block[B.np];
   int t = blockIdx.x;
   if (t >= ntiles) return;
-  // tile descriptors of this and the next tile of the CTA live in the 4 spare slots of the mbarrier area, the base
-  // address of the CTA's Tensor Memory in front of them
+  // 1-D block of NT compute threads (thread q = point (q % TX, q / TX % TY, q / (TX TY)) of the tile) + one producer warp
+  const int tid = threadIdx.x;
   TileId* desc = Src::desc();
-  uint32_t* tm_base = reinterpret_cast<uint32_t*>(tile_smem + C::BAR_OFF + 11);
-  static_assert(C::NS + 1 + C::RKD <= 11 && sizeof(TileId) == 16, "descriptor slots");
-  Src src;
-  src.maps = &M;
-  src.tid = threadIdx.x + C::TX * (threadIdx.y + C::TY * threadIdx.z);
-  if (src.tid == 0) {
-    desc[0] = locate<C>(B, t);
-    for (int i = 0; i < C::NS + 1 + C::RKD; ++i) tma::mbar_init(Src::bar(i), 1);
-    tma::fence_mbar_init();
+  uint32_t* tm_base = reinterpret_cast<uint32_t*>(tile_smem + C::TMB_OFF);
+  static_assert(sizeof(TileId) == 16, "descriptor slots");
+  if (tid == 0) {
+    desc[0] = locate_inl<C>(B, t);
+    Src::init_barriers();
   }
-  if (src.tid < 32) tmem::alloc_all(tm_base);   // warp 0 owns the allocation (and frees it at the end)
+  if (tid < 32) tmem::alloc_all(tm_base);   // warp 0 owns the allocation (and frees it at the end)
   tmem::fence_before_sync();
   __syncthreads();
   tmem::fence_after_sync();
-  TileId id = desc[0];
-  {
-    // the strip of this thread: Tensor Memory lane 32 (warp % 4) + lane, columns of warp / 4
-    const uint32_t warp = (uint32_t)src.tid / 32u;
-    src.tm = *tm_base + (((warp & 3u) * 32u) << 16) + (warp >> 2) * (2u * C::TM_DOUBLES);
-  }
-  src.iter = 0;
-  src.has_next = t + (int)gridDim.x < ntiles;
-  if (src.tid == 0) src.prime();   // loads of the first tile only: nxt is not needed yet
-  src.ey = C::EY_OFF + (threadIdx.z * C::TY + threadIdx.y) * C::EX + (threadIdx.x + 2);
-  src.ez = C::EZ_OFF + (threadIdx.z * (C::TY + 4) + (threadIdx.y + 2)) * C::EX + (threadIdx.x + 2);
-  src.xh = threadIdx.x < 2 ? -2 : (threadIdx.x >= C::TX - 2 ? 2 : 0);
-  src.yh = threadIdx.y < 2 ? -2 : 2;   // rows y-2 (y = 0, 1 -> -2, -1) and y+2 (y = 2, 3 -> TY, TY+1)
-  src.sc = ((threadIdx.z + NG) * C::PY + (threadIdx.y + NG)) * C::PX + (threadIdx.x + C::XC);
-
+  // The kernel starts with 65536 / NTH = 128 registers per thread; the producer warpgroup hands its registers to the
+  // compute warpgroups (a kernel that uses setmaxnreg must not contain calls: locate_inl)
+  if (tid >= C::NT) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::REG_PRODUCER));
+    if (tid == C::NT) Src::producer(&M, t, (int)gridDim.x, ntiles, [&](int tt) { return locate_inl<C>(B, tt); });
+  } else {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::REG_COMPUTE));
+    const int tx = tid % C::TX, ty = tid / C::TX % C::TY, tz = tid / (C::TX * C::TY);
+    Src src;
+    src.tid = tid;
+    {
+      // the strip of this thread: Tensor Memory lane 32 (warp % 4) + lane, columns of warp / 4
+      const uint32_t warp = (uint32_t)tid / 32u;
+      src.tm = *tm_base + (((warp & 3u) * 32u) << 16) + (warp >> 2) * (2u * C::TM_DOUBLES);
+    }
+    src.ey = C::EY_OFF + (tz * C::TY + ty) * C::EX + (tx + 2);
+    src.ez = C::EZ_OFF + (tz * (C::TY + 4) + (ty + 2)) * C::EX + (tx + 2);
+    src.xh = tx < 2 ? -2 : (tx >= C::TX - 2 ? 2 : 0);
+    src.yh = ty < 2 ? -2 : 2;   // rows y-2 (y = 0, 1 -> -2, -1) and y+2 (y = 2, 3 -> TY, TY+1)
+    src.sc = ((tz + NG) * C::PY + (ty + NG)) * C::PX + (tx + C::XC);
+    TileId id = desc[0];
 #pragma unroll 1
-  for (uint32_t iter = 0;; ++iter) {
-    const DevPatch& p = B.p[id.ip];
-    const int tn = t + gridDim.x;
-    src.has_next = tn < ntiles;
-    if (src.tid == 0 && src.has_next) desc[(iter + 1) & 1u] = locate<C>(B, tn);   // read by everybody after the barriers of this tile
-    src.iter = iter;
-    const int i = id.bx * C::TX + threadIdx.x, j = id.by * C::TY + threadIdx.y, k = id.bz * C::TZ + threadIdx.z;
-    const bool active = (i < p.nx) & (j < p.ny) & (k < p.nz);
-    const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
-    Emitter<(EPI < 0 ? 0 : EPI), Src> emit{src, rhs, rk.u_out, rk.acc, p.offset + c, p.fstride, p.dt, active};
-    src.begin_tile();
-    if constexpr (EPI < 0) constraints_point(src, p.dx, emit);
-    else z4c_point(src, P, p.dx, emit);
-    if (!src.has_next) break;
-    t = tn;
-    id = desc[(iter + 1) & 1u];   // written by thread 0 at the top of this tile, many barriers ago
+    for (uint32_t iter = 0;; ++iter) {
+      const DevPatch& p = B.p[id.ip];
+      const int tn = t + gridDim.x;
+      src.has_next = tn < ntiles;
+      src.iter = iter;
+      const int i = id.bx * C::TX + tx, j = id.by * C::TY + ty, k = id.bz * C::TZ + tz;
+      const bool active = (i < p.nx) & (j < p.ny) & (k < p.nz);
+      const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
+      Emitter<(EPI < 0 ? 0 : EPI), Src> emit{src, rhs, rk.u_out, rk.acc, p.offset + c, p.fstride, p.dt, active};
+      src.begin_tile();
+      if constexpr (EPI < 0) constraints_point(src, p.dx, emit);
+      else z4c_point(src, P, p.dx, emit);
+      if (!src.has_next) break;
+      t = tn;
+      id = desc[(iter + 1) & 1u];   // written by the producer at the top of this tile
+    }
   }
   tmem::fence_before_sync();
   __syncthreads();                // every thread is done with its strip
-  if (src.tid < 32) tmem::dealloc_all(*tm_base);
+  if (tid < 32) tmem::dealloc_all(*tm_base);
 }
 
 
@@ -536,7 +534,7 @@ static cudaError_t launch_one(int grid, cudaStream_t st, const PatchBatch& B, co
   static const cudaError_t attr =
       cudaFuncSetAttribute(k_z4c<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile::SMEM_BYTES);
   if (attr != cudaSuccess) return attr;
-  k_z4c<EPI><<<grid, dim3(Tile::TX, Tile::TY, Tile::TZ), Tile::SMEM_BYTES, st>>>(B, P, M, rhs, rk);
+  k_z4c<EPI><<<grid, Tile::NTH, Tile::SMEM_BYTES, st>>>(B, P, M, rhs, rk);
   return cudaGetLastError();
 }
 

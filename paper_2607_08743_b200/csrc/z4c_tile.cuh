@@ -146,7 +146,7 @@ struct TileCfg {
   // Tensor Memory: 512 columns shared by the warps of a lane quarter (warps w, w + 4, ...): doubles per thread
   static constexpr int TM_WARPS = (NT / 32 + 3) / 4;
   static constexpr int TM_DOUBLES = (512 / TM_WARPS) / 2 / 2 * 2;
-  static_assert(NT % 128 == 0 && PK_END <= TM_DOUBLES, "Tensor Memory strip of a thread");
+  static_assert(NT % 64 == 0 && PK_END <= TM_DOUBLES, "Tensor Memory strip of a thread");
   // box extents. x: the box must start on a 16-byte boundary of global memory (TMA rule for the innermost
   // coordinate, found by probing: an odd FP64 start coordinate raises "illegal instruction"); storage cell
   // bx*TX of a row sits at an odd double (sacra.h), so the box starts one cell earlier and is one cell wider
@@ -158,21 +158,32 @@ struct TileCfg {
   static constexpr int SLOT = (BOX + 15) / 16 * 16;            // doubles per ring slot (128-byte multiple)
   // shared-memory map (in doubles):
   //   ring | mbarriers | centre tile (NF x NT) | RK ring (RKD x {u_n, acc} x NT) | E_y | E_z
-  static constexpr int RKD = 5;                                // depth of the RK-input ring (divides NF)
-  static constexpr int BAR_OFF = NS * SLOT;                    // NS box + 1 centre + RKD rk mbarriers (16 reserved)
-  static constexpr int CEN_OFF = BAR_OFF + 16;                 // unpadded tiles of all NF fields
+  static constexpr int RKD = 8;                                // depth of the RK-input ring (a power of two)
+  static constexpr int NW = NT / 32;                           // compute warps of the CTA
+  // threads of the CTA: the compute warps + one producer warpgroup (setmaxnreg moves registers between whole
+  // warpgroups: the producer's three idle warps only donate theirs)
+  static constexpr int NTH = NT + 128;
+  static constexpr int REG_PRODUCER = 24;
+  static constexpr int REG_COMPUTE = (65536 - 128 * REG_PRODUCER) / NT / 8 * 8;
+  static_assert(NT % 128 == 0 && REG_COMPUTE >= 128 && REG_COMPUTE <= 255, "register split between the roles");
+  // mbarrier area (32 doubles): "full" NS box + 1 centre + RKD rk, "empty" NS box + 1 centre; then the base address of
+  // the CTA's Tensor Memory and two tile descriptors
+  static constexpr int BAR_OFF = NS * SLOT;
+  static constexpr int NBAR = 2 * NS + 2 + RKD;
+  static constexpr int TMB_OFF = BAR_OFF + NBAR;               // uint32 base address of the Tensor Memory allocation
+  static constexpr int DESC_OFF = BAR_OFF + 24;                // 2 x TileId (16 bytes each)
+  static constexpr int CEN_OFF = BAR_OFF + 32;                 // unpadded tiles of all NF fields
   static constexpr int CEN_BYTES = NF * NT * 8;
   static constexpr int RK_OFF = CEN_OFF + NF * NT;             // slot r: u_n tile at RK_OFF + 2 r NT, acc tile + NT
   static constexpr int EX = TX + 4;                            // x extent of the e arrays (x halo of 2)
   static constexpr int EY_OFF = RK_OFF + RKD * 2 * NT;         // e_y on  TZ x TY x (TX+4)
   static constexpr int EZ_OFF = EY_OFF + TZ * TY * EX;         // e_z on  TZ x (TY+4) x (TX+4)
   static constexpr int ESZ = TZ * TY * EX + TZ * (TY + 4) * EX;   // one set of e arrays
-  // with room for a second set of e arrays, fields with mixed derivatives need one block barrier instead of two
-  // (MERGE: the ring refill waits for the barrier of the e exchange; the sets alternate)
-  static constexpr bool MERGE = (EY_OFF + 2 * ESZ) * 8 + 1024 <= 233472;
-  static constexpr int SMEM_BYTES = (EY_OFF + (MERGE ? 2 : 1) * ESZ) * 8;
+  static constexpr int SMEM_BYTES = (EY_OFF + ESZ) * 8;
   static_assert(SMEM_BYTES + 1024 <= 233472, "shared memory of one SM");
-  static_assert(NF % RKD == 0 && NS + 2 + RKD <= 12, "mbarrier area / RK ring depth");
+  static_assert((RKD & (RKD - 1)) == 0 && NBAR < 24, "mbarrier area / RK ring depth");
+  static_assert(TX * TY == 64, "e exchange: one z-plane of the tile = two warps = one named barrier of 64 threads");
+  static_assert(TZ + 1 <= 15, "named barriers 1 .. TZ");
   static_assert(TY == 4 && TX >= 4, "e exchange: one y-halo row of e_z per thread row, x-halo columns by the edge lanes");
   static_assert((NT * 8) % 128 == 0 && SLOT % 16 == 0, "TMA destinations are 128-byte aligned");
   static_assert(NS >= 2 && NS <= 5, "ring depth");
@@ -183,21 +194,21 @@ struct TileCfg {
 // array (never through a stored generic pointer), so that every access compiles to LDS with an immediate offset.
 extern __shared__ __align__(1024) double tile_smem[];
 
-// barrier among the threads that exchange e values: the whole CTA (BAR = 0) or a named barrier of C::NT threads
-template <int BAR, int NTHREADS>
-__device__ __forceinline__ void group_sync() {
-  if constexpr (BAR == 0) __syncthreads();
-  else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(NTHREADS) : "memory");
+// Barrier among the threads that exchange e values. The mixed derivatives D_xy, D_xz, D_yz of a point need e_y / e_z
+// of points of the SAME z-plane only, and a z-plane of the tile is TX x TY = 64 threads = two warps: named barrier
+// 1 + z, 64 threads. No barrier of the kernel's tile loop spans the CTA: the warps of different planes drift apart by
+// up to NS - 1 fields (TileSource::field()), so that the stencil loads of one warp overlap the arithmetic of another.
+__device__ __forceinline__ void plane_sync() {   // 1-D block: thread t is point (t % TX, t / TX % TY, t / 64)
+  asm volatile("bar.sync %0, 64;" ::"r"(1u + threadIdx.x / 64u) : "memory");
 }
 
 // sample loader of one field for field_derivs(): shared-memory tile, compile-time strides
-template <class C, int BAR = 0, class Owner = void, int S = -1>
+template <class C>
 struct TileLoader {
   int c;       // index of this thread's centre inside the ring slot of the field
   int ey, ez;  // this thread's entries of the e arrays
   int xh;      // x-halo duty of this thread: 0 none, else the x offset (-2 or +2) of the column it also computes
   int yh;      // y offset (-2 or +2 rows... in units of rows) of the e_z y-halo entry this thread computes
-  const Owner* owner;   // MERGE: the tile source, told when the barrier of the e exchange has been passed
   __device__ __forceinline__ static constexpr int stride(int a) { return a == 0 ? 1 : (a == 1 ? C::PX : C::PX * C::PY); }
   __device__ __forceinline__ double operator()(int a, int k) const { return tile_smem[c + k * stride(a)]; }
   __device__ __forceinline__ double e_at(int o, int st) const {   // inner difference along stride st at centre + o
@@ -209,9 +220,11 @@ struct TileLoader {
   // axis b. e_y and e_z of a point are the numerators of its own D_y, D_z; every thread publishes its pair.
   // The entries two cells outside the tile are computed from the box without any table: thread row y computes
   // the e_z entry of y-halo row {-2, -1, TY, TY+1}[y] in its own column (TY = 4: one each), and the lanes of
-  // columns 0, 1 / TX-2, TX-1 compute e_y, e_z two columns to their left / right. One barrier, then the outer
+  // columns 0, 1 / TX-2, TX-1 compute e_y, e_z two columns to their left / right. Two barriers of the plane's two
+  // warps (one set of e arrays: the previous exchange has been read; this one has been written), then the outer
   // difference reads four neighbours.
   __device__ __forceinline__ void publish_e(double e_y, double e_z) const {
+    plane_sync();   // the partner warp has read the e values of the previous exchange
     tile_smem[ey] = e_y;
     tile_smem[ez] = e_z;
     tile_smem[ez + yh * C::EX] = e_at(yh * C::PX, C::PX * C::PY);
@@ -219,8 +232,7 @@ struct TileLoader {
       tile_smem[ey + xh] = e_at(xh, C::PX);
       tile_smem[ez + xh] = e_at(xh, C::PX * C::PY);
     }
-    group_sync<BAR, C::NT>();
-    if constexpr (!std::is_void<Owner>::value) owner->template after_publish<S>();
+    plane_sync();
   }
   __device__ __forceinline__ double e_y_x(int k) const { return tile_smem[ey + k]; }            // e_y at x + k
   __device__ __forceinline__ double e_z_x(int k) const { return tile_smem[ez + k]; }            // e_z at x + k
@@ -271,7 +283,6 @@ struct TileSource {
   uint32_t tm;             // Tensor Memory: address of double 0 of this thread's strip (a double = 2 columns)
   int ey, ez;              // shared memory: this thread's entries of the e arrays
   int xh, yh;              // halo duties of the e exchange (TileLoader)
-  const TileMaps* maps;    // kernel parameter (constant bank): costs no register
   bool has_next;
   uint32_t iter;           // tiles done by this CTA (ring phases)
 
@@ -279,11 +290,17 @@ struct TileSource {
   __device__ __forceinline__ static uint64_t* full(int slot) { return bar(slot); }            // box landed
   __device__ __forceinline__ static uint64_t* cen_full() { return bar(C::NS); }               // centre tile landed
   __device__ __forceinline__ static uint64_t* rk_full(int r) { return bar(C::NS + 1 + r); }   // RK inputs landed
+  // "empty" barriers, one arrival per warp: every warp is done with the ring slot / with the centre-value tile
+  __device__ __forceinline__ static uint64_t* empty(int slot) { return bar(C::NS + 1 + C::RKD + slot); }
+  __device__ __forceinline__ static uint64_t* cen_empty() { return bar(2 * C::NS + 1 + C::RKD); }
+  __device__ __forceinline__ static void init_barriers() {   // one thread
+    for (int i = 0; i < C::NS + 1 + C::RKD; ++i) tma::mbar_init(bar(i), 1);
+    for (int i = C::NS + 1 + C::RKD; i < C::NBAR; ++i) tma::mbar_init(bar(i), C::NW);
+    tma::fence_mbar_init();
+  }
 
-  // descriptors of this tile and of the CTA's next tile: two slots in shared memory, written by the leader (only the
-  // leader needs tile coordinates: they stay out of the registers of everybody else)
-  __device__ __forceinline__ static TileId* desc() { return reinterpret_cast<TileId*>(tile_smem + C::BAR_OFF + 12); }
-  __device__ __forceinline__ TileId tile(bool next) const { return desc()[(iter + (next ? 1u : 0u)) & 1u]; }
+  // descriptors of this tile and of the CTA's next tile: two slots in shared memory, written by the producer
+  __device__ __forceinline__ static TileId* desc() { return reinterpret_cast<TileId*>(tile_smem + C::DESC_OFF); }
   // map coordinates of the first active cell of a tile: map x coordinate c <-> storage cell c-1 (the maps start one
   // double before storage cell 0, on a 16-byte boundary), active cell i <-> storage cell i + NG
   __device__ __forceinline__ static int cx(const TileId& t) { return t.bx * C::TX + NG + 1; }
@@ -296,56 +313,112 @@ struct TileSource {
   __device__ __forceinline__ static uint32_t ring_slot(uint32_t it, int s) { return (it * Stream::N + s) % C::NS; }
   __device__ __forceinline__ static uint32_t ring_use(uint32_t it, int s) { return (it * Stream::N + s) / C::NS; }
 
-  // stream position S of tile `it` (S >= NF: position S - NF of tile it + 1, if there is one)
-  template <int S>
-  __device__ __forceinline__ void issue() const {
+  // ---- the producer's work (one lane of the extra warp): TMA requests with run-time field / slot numbers ----------
+  // stream position S of tile `it` (S >= N: position S - N of tile it + 1, if there is one)
+  __device__ __forceinline__ static void issue_box(const TileMaps* maps, uint32_t it, int S, bool has_next) {
     if (S >= Stream::N && !has_next) return;
-    constexpr int f = Stream::field(S % Stream::N);
-    const TileId t = tile(S >= Stream::N);
-    const uint32_t slot = ring_slot(iter, S);
+    const int f = stream_field_rt(S >= Stream::N ? S - Stream::N : S);
+    const TileId t = desc()[(it + (S >= Stream::N ? 1u : 0u)) & 1u];
+    const uint32_t slot = ring_slot(it, S);
     tma::mbar_expect_tx(full(slot), C::BOX_BYTES);
     // the box starts XC cells before the first active cell in x (an even map coordinate) and NG in y, z
     tma::load_box(tile_smem + slot * C::SLOT, &maps->box[t.ip], full(slot), cx(t) - C::XC, cy(t) - NG, cz(t) - NG, f,
                   tma::SACRA_BOX_POLICY);
   }
-  __device__ __forceinline__ void issue_centre(bool next) const {
-    const TileId t = tile(next);
+  __device__ __forceinline__ static void issue_centre(const TileMaps* maps, uint32_t it, bool next) {
+    const TileId t = desc()[(it + (next ? 1u : 0u)) & 1u];
     tma::mbar_expect_tx(cen_full(), C::CEN_BYTES);
     tma::load_box(tile_smem + C::CEN_OFF, &maps->cen[t.ip], cen_full(), cx(t), cy(t), cz(t), 0, tma::SACRA_CEN_POLICY);
   }
-  template <int E>
-  __device__ __forceinline__ void issue_rk(bool next) const {
-    constexpr int r = E % C::RKD, f = emit_field(E);
-    const TileId t = tile(next);
-    tma::mbar_expect_tx(rk_full(r), 2 * C::NT * 8);
-    tma::load_box(tile_smem + C::RK_OFF + 2 * r * C::NT, &maps->un[t.ip], rk_full(r), cx(t), cy(t), cz(t), f,
-                  tma::L2_EVICT_FIRST);
-    tma::load_box(tile_smem + C::RK_OFF + (2 * r + 1) * C::NT, &maps->acc[t.ip], rk_full(r), cx(t), cy(t), cz(t), f,
-                  tma::L2_EVICT_FIRST);
-  }
-  // RK inputs of emits (LO, HI]: emit indices >= NF belong to the next tile
-  template <int LO, int HI>
-  __device__ __forceinline__ void issue_rk_range() const {
-    if constexpr (LO < HI) {
-      constexpr int e = LO + 1;
-      if constexpr (e < NF) issue_rk<e>(false);
-      else if (has_next) issue_rk<e - NF>(true);
-      issue_rk_range<LO + 1, HI>();
+  // RK inputs of emits (lo, hi]: emit indices >= NF belong to the next tile
+  __device__ __forceinline__ static void issue_rk_range(const TileMaps* maps, uint32_t it, int lo, int hi, bool has_next) {
+#pragma unroll 1
+    for (int e = lo + 1; e <= hi; ++e) {
+      const bool next = e >= NF;
+      if (next && !has_next) return;
+      const int ee = next ? e - NF : e, f = emit_field_rt(ee);
+      const uint32_t r = (it * NF + (uint32_t)e) % C::RKD;     // ring position of emit sequence number it NF + e
+      const TileId t = desc()[(it + (next ? 1u : 0u)) & 1u];
+      tma::mbar_expect_tx(rk_full(r), 2 * C::NT * 8);
+      tma::load_box(tile_smem + C::RK_OFF + 2 * r * C::NT, &maps->un[t.ip], rk_full(r), cx(t), cy(t), cz(t), f,
+                    tma::L2_EVICT_FIRST);
+      tma::load_box(tile_smem + C::RK_OFF + (2 * r + 1) * C::NT, &maps->acc[t.ip], rk_full(r), cx(t), cy(t), cz(t), f,
+                    tma::L2_EVICT_FIRST);
     }
   }
-  // what the leader has in flight before the first field<>() call of a CTA
-  __device__ __forceinline__ void prime() const {
-    issue_centre(false);
-    issue<0>();
-    if constexpr (C::NS > 2) issue<1>();
-    if constexpr (C::NS > 3) issue<2>();
-    if constexpr (C::NS > 4) issue<3>();
-    if constexpr (RK == 2) issue_rk_range<-1, C::RKD - 2>();
+  // field of stream position s / of emit e for a run-time index: the orders packed 5 bits per entry into constants
+  template <class Fn>
+  __host__ __device__ static constexpr uint64_t pack5(Fn fn, int first, int n) {
+    uint64_t v = 0;
+    for (int q = 0; q < n; ++q) v |= (uint64_t)fn(first + q) << (5 * q);
+    return v;
+  }
+  __device__ __forceinline__ static int stream_field_rt(int sp) {
+    constexpr int n0 = Stream::N < 12 ? Stream::N : 12, n1 = Stream::N - n0 < 12 ? Stream::N - n0 : 12;
+    constexpr uint64_t a = pack5(Stream::field, 0, n0), b = pack5(Stream::field, 12, n1),
+                       c = pack5(Stream::field, 24, Stream::N - n0 - n1);
+    return (int)(((sp < 12 ? a >> (5 * sp) : sp < 24 ? b >> (5 * (sp - 12)) : c >> (5 * (sp - 24)))) & 31u);
+  }
+  __device__ __forceinline__ static int emit_field_rt(int e) {
+    constexpr uint64_t a = pack5(emit_field, 0, 12), b = pack5(emit_field, 12, 12), c = pack5(emit_field, 24, 1);
+    return (int)(((e < 12 ? a >> (5 * e) : e < 24 ? b >> (5 * (e - 12)) : c >> (5 * (e - 24)))) & 31u);
+  }
+  __device__ __forceinline__ static int emits_before_rt(int sp) {   // emits_before(sp), sp = 0 .. N
+    constexpr uint64_t a = pack5(emits_before, 0, 12), b = pack5(emits_before, 12, 12), c = pack5(emits_before, 24, 2);
+    return (int)(((sp < 12 ? a >> (5 * sp) : sp < 24 ? b >> (5 * (sp - 12)) : c >> (5 * (sp - 24)))) & 31u);
   }
 
+  // The PRODUCER: one lane of the CTA's extra warp owns every TMA request of the CTA. It walks the same sequence of
+  // tiles and stream positions as the compute warps; before stream position s of a tile it waits until every compute
+  // warp has released the ring slot of the previous position (NW arrivals on its "empty" barrier, made at the start
+  // of the warps' own field<>() call for s: every read of that slot and of the RK ring by the emits before s is
+  // behind them), then requests the box NS - 1 positions ahead into that slot and the RK inputs of the emits that
+  // may now be loaded. Tile descriptors: desc()[(it + 1) & 1] is written at the top of tile `it`, when every compute
+  // warp is inside tile it - 1 or later (it read that entry at the end of tile it - 2); the compute warps read it at
+  // the end of tile `it`, after many waits on "full" barriers armed later than the write.
+  template <class Locate>
+  __device__ __forceinline__ static void producer(const TileMaps* maps, int t, int stride, int ntiles, Locate locate) {
+    uint32_t it = 0;
+    bool has_next = t + stride < ntiles;
+    if (has_next) desc()[1] = locate(t + stride);
+    issue_centre(maps, it, false);
+#pragma unroll 1
+    for (int S = 0; S < C::NS - 1; ++S) issue_box(maps, it, S, has_next);
+    if constexpr (RK == 2) issue_rk_range(maps, it, -1, C::RKD - 2, has_next);
+#pragma unroll 1
+    for (;;) {
+#pragma unroll 1
+      for (int sp = 0; sp < Stream::N; ++sp) {
+        const uint32_t g = it * Stream::N + sp;
+        if (g > 0) tma::mbar_wait(empty((g - 1u) % C::NS), ((g - 1u) / C::NS) & 1u);
+        if (sp == 0 && has_next) {
+          tma::mbar_wait(cen_empty(), it & 1u);
+          issue_centre(maps, it, true);
+        }
+        issue_box(maps, it, sp + C::NS - 1, has_next);
+        if constexpr (RK == 2) {
+          // emit e may be loaded once emit e - RKD is done: through emits_before(sp) + RKD - 1
+          const int hi = emits_before_rt(sp) + C::RKD - 1;
+          const int lo = sp == 0 ? C::RKD - 2 : emits_before_rt(sp - 1) + C::RKD - 1;
+          issue_rk_range(maps, it, lo, hi, has_next);
+        }
+      }
+      if (!has_next) break;
+      t += stride;
+      ++it;
+      has_next = t + stride < ntiles;
+      if (has_next) desc()[(it + 1u) & 1u] = locate(t + stride);
+    }
+  }
+
+  // one arrival per warp on an "empty" barrier, after every lane's reads
+  __device__ __forceinline__ void warp_arrive(uint64_t* b) const {
+    __syncwarp();
+    if ((tid & 31) == 0) tma::mbar_arrive(b);
+  }
   // start of a tile: every thread copies its centre values from the shared-memory tile into its Tensor Memory strip
-  // (slot order of cen_slot()). After the first block barrier of the tile the buffer is free and the leader requests
-  // the next tile's values (refill<0>()).
+  // (slot order of cen_slot()). When every warp has done so the buffer is free and the producer requests the next
+  // tile's values.
   __device__ __forceinline__ void begin_tile() const {
     tma::mbar_wait(cen_full(), iter & 1u);
     const double* c = tile_smem + C::CEN_OFF + tid;
@@ -354,57 +427,25 @@ struct TileSource {
       tmem::st4(strip(q), c[cen_field(q) * C::NT], c[cen_field(q + 1) * C::NT], c[cen_field(q + 2) * C::NT],
                 c[cen_field(q + 3) * C::NT]);
     tmem::st1(strip(24), c[cen_field(24) * C::NT]);
+    warp_arrive(cen_empty());
     tmem::wait_st();
   }
 
-  // number of fields with mixed derivatives before stream position s (the e-array sets alternate between them)
-  __host__ __device__ static constexpr int d2_before(int s) {
-    int n = 0;
-    for (int q = 0; q < s; ++q) {
-      const int f = Stream::field(q);
-      if (f == F_W || (f >= F_G && f < F_G + 6) || f == F_ALP || (f >= F_BET && f < F_BET + 3)) ++n;
-    }
-    return n;
-  }
-  __host__ __device__ static constexpr bool is_d2(int f) {
-    return f == F_W || (f >= F_G && f < F_G + 6) || f == F_ALP || (f >= F_BET && f < F_BET + 3);
-  }
-  // leader: every thread is done with the slot of field s-1 and with every RK slot read so far -- refill them
-  template <int s>
-  __device__ __forceinline__ void refill() const {
-    if constexpr (s == 0) {
-      if (has_next) issue_centre(true);
-    }
-    issue<s + C::NS - 1>();
-    if constexpr (RK == 2) {
-      // emit e may be loaded once emit e - RKD is done: through emits_before(s) + RKD - 1
-      constexpr int hi = emits_before(s) + C::RKD - 1;
-      constexpr int lo = s == 0 ? C::RKD - 2 : emits_before(s - 1) + C::RKD - 1;
-      issue_rk_range<lo, hi>();
-    }
-  }
-  template <int s>
-  __device__ __forceinline__ void after_publish() const {
-    if (tid == 0) refill<s>();
-  }
-
+  // Advance to field F. No CTA-wide barrier: the warp releases the ring slot of the previous stream position (one
+  // arrival per warp on its "empty" barrier; program order puts every read of that slot, and every read of the RK
+  // ring by the emits so far, before it) and waits for the box of F. The producer refills a slot when all NW warps
+  // have released it, so a warp runs at most NS - 1 fields ahead of the slowest one.
   template <int F>
   __device__ __forceinline__ auto field() const {
     constexpr int s = Stream::slot(F);
     static_assert(s >= 0, "field not in this kernel's stream");
-    constexpr bool merged = C::MERGE && is_d2(F);
-    if constexpr (!merged) {
-      __syncthreads();
-      if (tid == 0) refill<s>();
+    const uint32_t g = iter * Stream::N + s;         // sequence number of this stream position in the CTA's ring
+    if (s > 0 || iter > 0) {
+      const uint32_t prev = g - 1u;
+      warp_arrive(empty(prev % C::NS));
     }
-    const uint32_t slot = ring_slot(iter, s);
-    tma::mbar_wait(full(slot), ring_use(iter, s) & 1u);
-    if constexpr (merged) {
-      constexpr int eo = (d2_before(s) & 1) * C::ESZ;
-      return TileLoader<C, 0, TileSource, s>{sc + (int)slot * C::SLOT, ey + eo, ez + eo, xh, yh, this};
-    } else {
-      return TileLoader<C>{sc + (int)slot * C::SLOT, ey, ez, xh, yh, nullptr};
-    }
+    tma::mbar_wait(full(g % C::NS), (g / C::NS) & 1u);
+    return TileLoader<C>{sc + (int)(g % C::NS) * C::SLOT, ey, ez, xh, yh};
   }
 
   // derivative bundle of field F: its tile from the ring, then the stencils
@@ -416,8 +457,9 @@ struct TileSource {
   // RK inputs of field F at this point (stages 2-4): waits for the ring slot of its emit
   template <int F>
   __device__ __forceinline__ void rk_inputs(double& un, double& acc) const {
-    constexpr int e = emit_slot(F), r = e % C::RKD;
-    tma::mbar_wait(rk_full(r), (iter * (NF / C::RKD) + e / C::RKD) & 1u);
+    constexpr int e = emit_slot(F);
+    const uint32_t q = iter * NF + e, r = q % C::RKD;          // emit sequence number of the CTA, ring position
+    tma::mbar_wait(rk_full(r), (q / C::RKD) & 1u);
     un = tile_smem[C::RK_OFF + 2 * r * C::NT + tid];
     acc = tile_smem[C::RK_OFF + (2 * r + 1) * C::NT + tid];
   }
