@@ -178,9 +178,9 @@ struct Emitter {
 // slab of 25 fields is 131 MB): 28.8 GB read per launch against 6.7 GB algorithmic.
 // Only thread 0 decodes tile indices (several integer divisions); the CTA gets them through shared memory.
 #ifndef SACRA_SBX
-#define SACRA_SBX 4
-#define SACRA_SBY 16
-#define SACRA_SBZ 8
+#define SACRA_SBX 16
+#define SACRA_SBY 4
+#define SACRA_SBZ 4
 #endif
 #ifndef SACRA_L2PROMO
 #define SACRA_L2PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_128B
@@ -240,7 +240,8 @@ __global__ void __launch_bounds__(Tile::NTH, 1) k_z4c(const __grid_constant__ Pa
   // compute warpgroups (a kernel that uses setmaxnreg must not contain calls: locate_inl)
   if (tid >= C::NT) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::REG_PRODUCER));
-    if (tid == C::NT) Src::producer(&M, t, (int)gridDim.x, ntiles, [&](int tt) { return locate_inl<C>(B, tt); });
+    if (tid % 32 == 0 && tid < C::NT + 96)
+      Src::producer((tid - C::NT) / 32, &M, t, (int)gridDim.x, ntiles, [&](int tt) { return locate_inl<C>(B, tt); });
   } else {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::REG_COMPUTE));
     const int tx = tid % C::TX, ty = tid / C::TX % C::TY, tz = tid / (C::TX * C::TY);

@@ -139,6 +139,9 @@ constexpr int PK_AUU = 64;   // At^ij,      3 groups i of 4 doubles (j = 0..2, p
 constexpr int PK_AG = 76;    // advection and KO of Gt^k, 3 groups k of 2 doubles
 constexpr int PK_END = 82;
 
+#ifndef SACRA_RKD
+#define SACRA_RKD 8
+#endif
 template <int TX_, int TY_, int TZ_, int NS_>
 struct TileCfg {
   static constexpr int TX = TX_, TY = TY_, TZ = TZ_, NS = NS_;
@@ -158,20 +161,20 @@ struct TileCfg {
   static constexpr int SLOT = (BOX + 15) / 16 * 16;            // doubles per ring slot (128-byte multiple)
   // shared-memory map (in doubles):
   //   ring | mbarriers | centre tile (NF x NT) | RK ring (RKD x {u_n, acc} x NT) | E_y | E_z
-  static constexpr int RKD = 8;                                // depth of the RK-input ring (a power of two)
+  static constexpr int RKD = SACRA_RKD;                               // depth of the RK-input ring (a power of two)
   static constexpr int NW = NT / 32;                           // compute warps of the CTA
   // threads of the CTA: the compute warps + one producer warpgroup (setmaxnreg moves registers between whole
   // warpgroups: the producer's three idle warps only donate theirs)
   static constexpr int NTH = NT + 128;
-  static constexpr int REG_PRODUCER = 24;
+  static constexpr int REG_PRODUCER = 32;
   static constexpr int REG_COMPUTE = (65536 - 128 * REG_PRODUCER) / NT / 8 * 8;
   static_assert(NT % 128 == 0 && REG_COMPUTE >= 128 && REG_COMPUTE <= 255, "register split between the roles");
-  // mbarrier area (32 doubles): "full" NS box + 1 centre + RKD rk, "empty" NS box + 1 centre; then the base address of
-  // the CTA's Tensor Memory and two tile descriptors
+  // mbarrier area (32 doubles): "full" NS box + 1 centre + RKD rk, "empty" NS box + 1 centre + RKD rk; then the base
+  // address of the CTA's Tensor Memory and two tile descriptors
   static constexpr int BAR_OFF = NS * SLOT;
-  static constexpr int NBAR = 2 * NS + 2 + RKD;
+  static constexpr int NBAR = 2 * NS + 2 + 2 * RKD;
   static constexpr int TMB_OFF = BAR_OFF + NBAR;               // uint32 base address of the Tensor Memory allocation
-  static constexpr int DESC_OFF = BAR_OFF + 24;                // 2 x TileId (16 bytes each)
+  static constexpr int DESC_OFF = BAR_OFF + 28;                // 2 x TileId (16 bytes each)
   static constexpr int CEN_OFF = BAR_OFF + 32;                 // unpadded tiles of all NF fields
   static constexpr int CEN_BYTES = NF * NT * 8;
   static constexpr int RK_OFF = CEN_OFF + NF * NT;             // slot r: u_n tile at RK_OFF + 2 r NT, acc tile + NT
@@ -181,7 +184,7 @@ struct TileCfg {
   static constexpr int ESZ = TZ * TY * EX + TZ * (TY + 4) * EX;   // one set of e arrays
   static constexpr int SMEM_BYTES = (EY_OFF + ESZ) * 8;
   static_assert(SMEM_BYTES + 1024 <= 233472, "shared memory of one SM");
-  static_assert((RKD & (RKD - 1)) == 0 && NBAR < 24, "mbarrier area / RK ring depth");
+  static_assert((RKD & (RKD - 1)) == 0 && NBAR < 28, "mbarrier area / RK ring depth");
   static_assert(TX * TY == 64, "e exchange: one z-plane of the tile = two warps = one named barrier of 64 threads");
   static_assert(TZ + 1 <= 15, "named barriers 1 .. TZ");
   static_assert(TY == 4 && TX >= 4, "e exchange: one y-halo row of e_z per thread row, x-halo columns by the edge lanes");
@@ -293,9 +296,11 @@ struct TileSource {
   // "empty" barriers, one arrival per warp: every warp is done with the ring slot / with the centre-value tile
   __device__ __forceinline__ static uint64_t* empty(int slot) { return bar(C::NS + 1 + C::RKD + slot); }
   __device__ __forceinline__ static uint64_t* cen_empty() { return bar(2 * C::NS + 1 + C::RKD); }
+  __device__ __forceinline__ static uint64_t* rk_empty(int r) { return bar(2 * C::NS + 2 + C::RKD + r); }
   __device__ __forceinline__ static void init_barriers() {   // one thread
-    for (int i = 0; i < C::NS + 1 + C::RKD; ++i) tma::mbar_init(bar(i), 1);
-    for (int i = C::NS + 1 + C::RKD; i < C::NBAR; ++i) tma::mbar_init(bar(i), C::NW);
+    for (int i = 0; i < C::NS + 1; ++i) tma::mbar_init(bar(i), 1);
+    for (int i = C::NS + 1; i < C::NS + 1 + C::RKD; ++i) tma::mbar_init(bar(i), 2);   // the u_n and the acc producer
+    for (int i = C::NS + 1 + C::RKD; i < C::NBAR; ++i) tma::mbar_init(bar(i), C::NW);   // "empty": one arrival per warp
     tma::fence_mbar_init();
   }
 
@@ -313,38 +318,27 @@ struct TileSource {
   __device__ __forceinline__ static uint32_t ring_slot(uint32_t it, int s) { return (it * Stream::N + s) % C::NS; }
   __device__ __forceinline__ static uint32_t ring_use(uint32_t it, int s) { return (it * Stream::N + s) / C::NS; }
 
-  // ---- the producer's work (one lane of the extra warp): TMA requests with run-time field / slot numbers ----------
-  // stream position S of tile `it` (S >= N: position S - N of tile it + 1, if there is one)
-  __device__ __forceinline__ static void issue_box(const TileMaps* maps, uint32_t it, int S, bool has_next) {
-    if (S >= Stream::N && !has_next) return;
+  // ---- the producers' work: TMA requests with run-time field / slot numbers ---------------------------------------
+  // stream position S of tile `it` (S >= N: position S - N of tile it + 1, whose descriptor is `t`)
+  __device__ __forceinline__ static void issue_box(const TileMaps* maps, uint32_t it, int S, const TileId& t) {
     const int f = stream_field_rt(S >= Stream::N ? S - Stream::N : S);
-    const TileId t = desc()[(it + (S >= Stream::N ? 1u : 0u)) & 1u];
     const uint32_t slot = ring_slot(it, S);
     tma::mbar_expect_tx(full(slot), C::BOX_BYTES);
     // the box starts XC cells before the first active cell in x (an even map coordinate) and NG in y, z
     tma::load_box(tile_smem + slot * C::SLOT, &maps->box[t.ip], full(slot), cx(t) - C::XC, cy(t) - NG, cz(t) - NG, f,
                   tma::SACRA_BOX_POLICY);
   }
-  __device__ __forceinline__ static void issue_centre(const TileMaps* maps, uint32_t it, bool next) {
-    const TileId t = desc()[(it + (next ? 1u : 0u)) & 1u];
+  __device__ __forceinline__ static void issue_centre(const TileMaps* maps, const TileId& t) {
     tma::mbar_expect_tx(cen_full(), C::CEN_BYTES);
     tma::load_box(tile_smem + C::CEN_OFF, &maps->cen[t.ip], cen_full(), cx(t), cy(t), cz(t), 0, tma::SACRA_CEN_POLICY);
   }
-  // RK inputs of emits (lo, hi]: emit indices >= NF belong to the next tile
-  __device__ __forceinline__ static void issue_rk_range(const TileMaps* maps, uint32_t it, int lo, int hi, bool has_next) {
-#pragma unroll 1
-    for (int e = lo + 1; e <= hi; ++e) {
-      const bool next = e >= NF;
-      if (next && !has_next) return;
-      const int ee = next ? e - NF : e, f = emit_field_rt(ee);
-      const uint32_t r = (it * NF + (uint32_t)e) % C::RKD;     // ring position of emit sequence number it NF + e
-      const TileId t = desc()[(it + (next ? 1u : 0u)) & 1u];
-      tma::mbar_expect_tx(rk_full(r), 2 * C::NT * 8);
-      tma::load_box(tile_smem + C::RK_OFF + 2 * r * C::NT, &maps->un[t.ip], rk_full(r), cx(t), cy(t), cz(t), f,
-                    tma::L2_EVICT_FIRST);
-      tma::load_box(tile_smem + C::RK_OFF + (2 * r + 1) * C::NT, &maps->acc[t.ip], rk_full(r), cx(t), cy(t), cz(t), f,
-                    tma::L2_EVICT_FIRST);
-    }
+  // RK input `which` (0: u_n, 1: acc) of emit e of tile t, the CTA's emit number q
+  __device__ __forceinline__ static void issue_rk(const CUtensorMap* map, int which, uint32_t q, int e, const TileId& t) {
+    const int f = emit_field_rt(e);
+    const uint32_t r = q % C::RKD;
+    tma::mbar_expect_tx(rk_full(r), C::NT * 8);
+    tma::load_box(tile_smem + C::RK_OFF + (2 * r + which) * C::NT, map + t.ip, rk_full(r), cx(t), cy(t), cz(t), f,
+                  tma::L2_EVICT_FIRST);
   }
   // field of stream position s / of emit e for a run-time index: the orders packed 5 bits per entry into constants
   template <class Fn>
@@ -363,51 +357,66 @@ struct TileSource {
     constexpr uint64_t a = pack5(emit_field, 0, 12), b = pack5(emit_field, 12, 12), c = pack5(emit_field, 24, 1);
     return (int)(((e < 12 ? a >> (5 * e) : e < 24 ? b >> (5 * (e - 12)) : c >> (5 * (e - 24)))) & 31u);
   }
-  __device__ __forceinline__ static int emits_before_rt(int sp) {   // emits_before(sp), sp = 0 .. N
-    constexpr uint64_t a = pack5(emits_before, 0, 12), b = pack5(emits_before, 12, 12), c = pack5(emits_before, 24, 2);
-    return (int)(((sp < 12 ? a >> (5 * sp) : sp < 24 ? b >> (5 * (sp - 12)) : c >> (5 * (sp - 24)))) & 31u);
-  }
-
-  // The PRODUCER: one lane of the CTA's extra warp owns every TMA request of the CTA. It walks the same sequence of
-  // tiles and stream positions as the compute warps; before stream position s of a tile it waits until every compute
-  // warp has released the ring slot of the previous position (NW arrivals on its "empty" barrier, made at the start
-  // of the warps' own field<>() call for s: every read of that slot and of the RK ring by the emits before s is
-  // behind them), then requests the box NS - 1 positions ahead into that slot and the RK inputs of the emits that
-  // may now be loaded. Tile descriptors: desc()[(it + 1) & 1] is written at the top of tile `it`, when every compute
-  // warp is inside tile it - 1 or later (it read that entry at the end of tile it - 2); the compute warps read it at
-  // the end of tile `it`, after many waits on "full" barriers armed later than the write.
+  // The PRODUCERS: one lane each of up to three warps of the CTA's extra warpgroup owns the TMA requests of the CTA --
+  // role 0 the stencil boxes and the centre-value tile, roles 1 and 2 (RK stages 2-4) the u_n and the acc tile of
+  // every emit, so that the ~150 cycles one request costs its issuing thread are not spent in series. Each is a plain
+  // ring producer: it walks the CTA's sequence of tiles and stream positions (emits), and before it refills a slot it
+  // waits for the NW arrivals of the compute warps on the slot's "empty" barrier (box ring: made at the start of the
+  // warps' field<>() call for the next position; RK ring: right after the emit has read its inputs). Every producer
+  // waits for every phase of its barriers in order, and a phase cannot complete before the producer has filled the
+  // slot for it, so the parity waits never alias.
+  // Tile descriptors stay in the producers' registers; role 0 publishes them to the compute warps:
+  // desc()[(it + 1) & 1] is written at the top of tile `it`, when every compute warp is inside tile it - 1 or later (it
+  // read that entry at the end of tile it - 2); the compute warps read it at the end of tile `it`, after many waits
+  // on "full" barriers armed later than the write.
   template <class Locate>
-  __device__ __forceinline__ static void producer(const TileMaps* maps, int t, int stride, int ntiles, Locate locate) {
+  __device__ __forceinline__ static void producer(int role, const TileMaps* maps, int t, int stride, int ntiles,
+                                                  Locate locate) {
+    if (RK != 2 && role != 0) return;
     uint32_t it = 0;
+    TileId cur = desc()[0], nxt = cur;
     bool has_next = t + stride < ntiles;
-    if (has_next) desc()[1] = locate(t + stride);
-    issue_centre(maps, it, false);
+    if (role == 0) {
+      if (has_next) desc()[1] = nxt = locate(t + stride);
+      issue_centre(maps, cur);
 #pragma unroll 1
-    for (int S = 0; S < C::NS - 1; ++S) issue_box(maps, it, S, has_next);
-    if constexpr (RK == 2) issue_rk_range(maps, it, -1, C::RKD - 2, has_next);
+      for (int S = 0; S < C::NS - 1; ++S) issue_box(maps, it, S, cur);
 #pragma unroll 1
-    for (;;) {
+      for (;;) {
 #pragma unroll 1
-      for (int sp = 0; sp < Stream::N; ++sp) {
-        const uint32_t g = it * Stream::N + sp;
-        if (g > 0) tma::mbar_wait(empty((g - 1u) % C::NS), ((g - 1u) / C::NS) & 1u);
-        if (sp == 0 && has_next) {
-          tma::mbar_wait(cen_empty(), it & 1u);
-          issue_centre(maps, it, true);
+        for (int sp = 0; sp < Stream::N; ++sp) {
+          const uint32_t g = it * Stream::N + sp;
+          if (g > 0) tma::mbar_wait(empty((g - 1u) % C::NS), ((g - 1u) / C::NS) & 1u);
+          if (sp == 0 && has_next) {
+            tma::mbar_wait(cen_empty(), it & 1u);
+            issue_centre(maps, nxt);
+          }
+          const int S = sp + C::NS - 1;
+          if (S < Stream::N) issue_box(maps, it, S, cur);
+          else if (has_next) issue_box(maps, it, S, nxt);
         }
-        issue_box(maps, it, sp + C::NS - 1, has_next);
-        if constexpr (RK == 2) {
-          // emit e may be loaded once emit e - RKD is done: through emits_before(sp) + RKD - 1
-          const int hi = emits_before_rt(sp) + C::RKD - 1;
-          const int lo = sp == 0 ? C::RKD - 2 : emits_before_rt(sp - 1) + C::RKD - 1;
-          issue_rk_range(maps, it, lo, hi, has_next);
-        }
+        if (!has_next) break;
+        t += stride;
+        ++it;
+        cur = nxt;
+        has_next = t + stride < ntiles;
+        if (has_next) desc()[(it + 1u) & 1u] = nxt = locate(t + stride);
       }
-      if (!has_next) break;
-      t += stride;
-      ++it;
-      has_next = t + stride < ntiles;
-      if (has_next) desc()[(it + 1u) & 1u] = locate(t + stride);
+    } else {
+      const CUtensorMap* map = role == 1 ? maps->un : maps->acc;
+      uint32_t q = 0;                                           // emit number of the CTA
+#pragma unroll 1
+      for (;;) {
+#pragma unroll 1
+        for (int e = 0; e < NF; ++e, ++q) {
+          if (q >= (uint32_t)C::RKD) tma::mbar_wait(rk_empty(q % C::RKD), (q / C::RKD - 1u) & 1u);
+          issue_rk(map, role - 1, q, e, cur);
+        }
+        if (!has_next) break;
+        t += stride;
+        cur = locate(t);
+        has_next = t + stride < ntiles;
+      }
     }
   }
 
@@ -462,6 +471,7 @@ struct TileSource {
     tma::mbar_wait(rk_full(r), (q / C::RKD) & 1u);
     un = tile_smem[C::RK_OFF + 2 * r * C::NT + tid];
     acc = tile_smem[C::RK_OFF + (2 * r + 1) * C::NT + tid];
+    warp_arrive(rk_empty(r));
   }
 };
 
