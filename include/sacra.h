@@ -68,8 +68,14 @@ typedef struct {
   double ko_sigma;         /* Kreiss-Oliger strength; Q = sigma h^5/64 (D+D-)^3       */
   int32_t lapse_uses_khat; /* Eq. 6 source: 1 -> -2 alpha K-hat (default reading),
                               0 -> -2 alpha (K-hat + 2 Theta)                                       */
-  int32_t reserved_;       /* set to 0                                                              */
+  int32_t flags;           /* 0, or SACRA_FLAG_* values or'ed together                               */
 } sacra_params_t;
+
+/* sacra_params_t.flags */
+#define SACRA_FLAG_SKIP_INCREMENT 1 /* stage 4 of the RK4 step does not store the increment S to acc (SURVEY 8(c)
+                                       item 11: "this write may be skipped outside verification"): one field pass
+                                       less per step; the contents of acc are then unspecified after stage 4 / after
+                                       sacra_rk4_step. u_out is the same bit for bit.                             */
 
 /* Periodic halo fill (stands in for the paper's ghost exchange).
  * For every field of every patch, each storage cell with an index outside the active range takes the
@@ -101,7 +107,10 @@ int sacra_z4c_rhs(const sacra_patch_t* p, int npatch, const sacra_params_t* prm,
  *   stage 4: S = (acc + k) * (1/6)  ; u_out = u_n + dt S ; acc = S
  * u_in: ghosts filled (read through the stencil). u_n: read at active cells only. u_out, acc: active
  * cells written, ghosts not touched. u_out must not alias u_in; u_out may alias u_n (centre-only access);
- * acc must alias none of the others. At stage 1 acc is write-only. */
+ * acc must alias none of the others. At stage 1 acc is write-only.
+ * Aliasing is checked on whole states: any two of the four buffers must either be the same pointer, where the table
+ * allows it (u_n = u_in, required at stage 1; u_out = u_n), or disjoint address ranges of the extent the patch
+ * descriptors span -- a partial overlap returns SACRA_ERR_BADARG, like every other forbidden aliasing. */
 int sacra_rk4_substep(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, int stage,
                       const double* u_n, const double* u_in, double* u_out, double* acc,
                       void* cuda_stream);
@@ -109,8 +118,10 @@ int sacra_rk4_substep(const sacra_patch_t* p, int npatch, const sacra_params_t* 
 /* One full RK4 step: for s = 1..4 { fill_ghosts(stage input); rk4_substep(s) }; fill_ghosts(result).
  * u: in = state n (ghosts need not be filled), out = state n+1 with ghosts filled.
  * work: 3 states back to back, each `state_doubles` long (two stage buffers and acc). On return
- * work + 2*state_doubles holds S, the increment per unit dt, on active cells. Bitwise identical to the
- * nine-call sequence above. */
+ * work + 2*state_doubles holds S, the increment per unit dt, on active cells (unless prm->flags has
+ * SACRA_FLAG_SKIP_INCREMENT). Bitwise identical to the nine-call sequence above. u must not overlap
+ * [work, work + 3*state_doubles). Every call of the library only enqueues kernels on cuda_stream, so a step can be
+ * captured into a CUDA graph by the caller (the tiny configurations are launch-bound: bench.py --all-configs). */
 int sacra_rk4_step(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, double* u,
                    double* work, int64_t state_doubles, void* cuda_stream);
 
@@ -143,7 +154,7 @@ int64_t sacra_constraint_scratch_doubles(const sacra_patch_t* p, int npatch);
  *                         axis Lagrange interpolant of the parent data at its centre (a quarter of a parent spacing
  *                         off the parent cell that holds it). Parent cells org + floor(i/2) - 3 .. + 3 are read for
  *                         child cells i = -3 .. n+2: they must lie in the parent's storage (ghosts included, valid).
- * Time interpolation and the subcycling driver are not part of the library. */
+ * The child's spacing must be half the parent's; the two states must not overlap. */
 int sacra_restrict(const sacra_patch_t* parent, const sacra_patch_t* child, const int32_t* org, double* u_parent,
                    const double* u_child, void* cuda_stream);
 int sacra_prolong_ghosts(const sacra_patch_t* parent, const sacra_patch_t* child, const int32_t* org,

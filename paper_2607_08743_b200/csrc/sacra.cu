@@ -9,6 +9,7 @@
 // There is no CPU path: every entry point enqueues kernels on the caller's stream or returns an error.
 #include <cmath>
 #include <cstdint>
+#include <mutex>
 #include <cuda_runtime.h>
 #include <type_traits>
 
@@ -117,7 +118,7 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
 #endif
 using Tile = TileCfg<SACRA_TX, SACRA_TY, SACRA_TZ, SACRA_NS>;
 
-// EPI: 0 = store RHS; 1..4 = RK4 substage (item 11 table)
+// EPI: 0 = store RHS; 1..4 = RK4 substage (item 11 table); 5 = substage 4 without the store of the increment S
 struct RkArgs {
   const double* u_n;
   double* u_out;
@@ -159,12 +160,12 @@ struct Emitter {
     } else if (EPI == 3) {
       acc_new = __dadd_rn(ac, __dmul_rn(2.0, kk));
       u_new = __dadd_rn(un, __dmul_rn(dt, kk));
-    } else {
+    } else {   // stage 4; EPI 5: the same without the store of S (SACRA_FLAG_SKIP_INCREMENT)
       acc_new = __dmul_rn(__dadd_rn(ac, kk), 1.0 / 6.0);
       u_new = __dadd_rn(un, __dmul_rn(dt, acc_new));
     }
     if (active) {
-      __stcs(acc + a, acc_new);   // streaming stores: they must not evict the stencil boxes from L2
+      if (EPI != 5) __stcs(acc + a, acc_new);   // streaming stores: they must not evict the stencil boxes from L2
       __stcs(u_out + a, u_new);
     }
   }
@@ -447,6 +448,22 @@ static int check_patches(const sacra_patch_t* p, int npatch) {
   return SACRA_OK;
 }
 
+// doubles from a state's base pointer to the end of its last patch
+static long long state_extent(const sacra_patch_t* p, int npatch) {
+  long long ext = 0;
+  for (int q = 0; q < npatch; ++q) {
+    const long long need = (long long)p[q].pitch_x * (p[q].ny + 2 * SACRA_NG) * (p[q].nz + 2 * SACRA_NG);
+    const long long e = p[q].patch_offset + (long long)(SACRA_NF - 1) * p[q].field_stride + need;
+    if (e > ext) ext = e;
+  }
+  return ext;
+}
+// do [a, a + na) and [b, b + nb) (in doubles) share a byte?
+static bool overlap(const double* a, long long na, const double* b, long long nb) {
+  const uintptr_t a0 = reinterpret_cast<uintptr_t>(a), b0 = reinterpret_cast<uintptr_t>(b);
+  return a0 < b0 + (uintptr_t)nb * 8u && b0 < a0 + (uintptr_t)na * 8u;
+}
+
 static DevPatch to_dev(const sacra_patch_t& a) {
   DevPatch d;
   d.nx = a.nx; d.ny = a.ny; d.nz = a.nz;
@@ -518,21 +535,54 @@ static int make_map(const sacra_patch_t& a, const double* u, int bx, int by, int
   return r == CUDA_SUCCESS ? SACRA_OK : SACRA_ERR_CUDA;
 }
 
+// Encoding a tensor map costs a few microseconds on the host and a substage launch needs 2-4 per patch, which is most
+// of the cost of a step on the small configurations. A map depends only on (address, layout, box), and callers step
+// the same buffers over and over: keep the last MAPCACHE maps (a tensor map holds no device state; it stays valid as
+// long as the address range it describes is what the caller passes again).
+struct MapKey {
+  const void* base;
+  long long pitch, fstride;
+  int nx, ny, nz, bx, by, bz, bf;
+  bool operator==(const MapKey& o) const {
+    return base == o.base && pitch == o.pitch && fstride == o.fstride && nx == o.nx && ny == o.ny && nz == o.nz &&
+           bx == o.bx && by == o.by && bz == o.bz && bf == o.bf;
+  }
+};
+constexpr int MAPCACHE = 256;
+static std::mutex map_mutex;
+static MapKey map_keys[MAPCACHE];
+static CUtensorMap map_vals[MAPCACHE];
+static int map_count = 0, map_next = 0;
+
+static int cached_map(const sacra_patch_t& a, const double* u, int bx, int by, int bz, int bf, CUtensorMap* out) {
+  const MapKey k{u + a.patch_offset, a.pitch_x, a.field_stride, a.nx, a.ny, a.nz, bx, by, bz, bf};
+  std::lock_guard<std::mutex> lock(map_mutex);
+  for (int i = 0; i < map_count; ++i)
+    if (map_keys[i] == k) {
+      *out = map_vals[i];
+      return SACRA_OK;
+    }
+  if (int e = make_map(a, u, bx, by, bz, bf, out)) return e;
+  const int slot = map_count < MAPCACHE ? map_count++ : (map_next++ % MAPCACHE);
+  map_keys[slot] = k;
+  map_vals[slot] = *out;
+  return SACRA_OK;
+}
+
+// per-device facts are asked for at every launch (one process may drive several devices)
 static int num_sms() {
-  static int n = [] {
-    int dev = 0, v = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
-    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
-    return v;
-  }();
-  return n;
+  int dev = 0, v = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+  if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+  return v;
 }
 
 
 template <int EPI>
 static cudaError_t launch_one(int grid, cudaStream_t st, const PatchBatch& B, const Params& P, const TileMaps& M,
                               double* rhs, const RkArgs& rk) {
-  static const cudaError_t attr =
+  // the opt-in to > 48 KB of dynamic shared memory is per device: set it at every launch (a host-side table lookup)
+  const cudaError_t attr =
       cudaFuncSetAttribute(k_z4c<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Tile::SMEM_BYTES);
   if (attr != cudaSuccess) return attr;
   k_z4c<EPI><<<grid, Tile::NTH, Tile::SMEM_BYTES, st>>>(B, P, M, rhs, rk);
@@ -556,11 +606,11 @@ static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* 
       B.p[q] = to_dev(a);
       B.first_block[q] = nb;
       nb += ((a.nx + Tile::TX - 1) / Tile::TX) * ((a.ny + Tile::TY - 1) / Tile::TY) * ((a.nz + Tile::TZ - 1) / Tile::TZ);
-      if (int e = make_map(a, u_in, Tile::PX, Tile::PY, Tile::PZ, 1, &M.box[q])) return e;
-      if (int e = make_map(a, u_in, Tile::TX, Tile::TY, Tile::TZ, NF, &M.cen[q])) return e;
+      if (int e = cached_map(a, u_in, Tile::PX, Tile::PY, Tile::PZ, 1, &M.box[q])) return e;
+      if (int e = cached_map(a, u_in, Tile::TX, Tile::TY, Tile::TZ, NF, &M.cen[q])) return e;
       if (epi >= 2) {
-        if (int e = make_map(a, u_n, Tile::TX, Tile::TY, Tile::TZ, 1, &M.un[q])) return e;
-        if (int e = make_map(a, acc, Tile::TX, Tile::TY, Tile::TZ, 1, &M.acc[q])) return e;
+        if (int e = cached_map(a, u_n, Tile::TX, Tile::TY, Tile::TZ, 1, &M.un[q])) return e;
+        if (int e = cached_map(a, acc, Tile::TX, Tile::TY, Tile::TZ, 1, &M.acc[q])) return e;
       }
     }
     B.first_block[B.np] = nb;
@@ -572,7 +622,8 @@ static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* 
       case 1: err = launch_one<1>(grid, st, B, P, M, rhs, rk); break;
       case 2: err = launch_one<2>(grid, st, B, P, M, rhs, rk); break;
       case 3: err = launch_one<3>(grid, st, B, P, M, rhs, rk); break;
-      default: err = launch_one<4>(grid, st, B, P, M, rhs, rk); break;
+      case 4: err = launch_one<4>(grid, st, B, P, M, rhs, rk); break;
+      default: err = launch_one<5>(grid, st, B, P, M, rhs, rk); break;
     }
     if (err != cudaSuccess) return SACRA_ERR_CUDA;
   }
@@ -609,7 +660,8 @@ int sacra_z4c_rhs(const sacra_patch_t* p, int npatch, const sacra_params_t* prm,
   if (!p || !prm || !u || !rhs) return SACRA_ERR_NULL;
   if (int e = check_patches(p, npatch)) return e;
   if (!aligned16(u) || !aligned16(rhs)) return SACRA_ERR_ALIGN;
-  if (u == rhs) return SACRA_ERR_BADARG;
+  const long long ext = state_extent(p, npatch);
+  if (overlap(u, ext, rhs, ext)) return SACRA_ERR_BADARG;
   return launch_z4c(p, npatch, prm, 0, u, rhs, nullptr, nullptr, nullptr, static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -619,8 +671,16 @@ int sacra_rk4_substep(const sacra_patch_t* p, int npatch, const sacra_params_t* 
   if (int e = check_patches(p, npatch)) return e;
   if (stage < 1 || stage > 4) return SACRA_ERR_BADARG;
   if (!aligned16(u_n) || !aligned16(u_in) || !aligned16(u_out) || !aligned16(acc)) return SACRA_ERR_ALIGN;
-  if (u_out == u_in || acc == u_in || acc == u_n || acc == u_out) return SACRA_ERR_BADARG;
-  return launch_z4c(p, npatch, prm, stage, u_in, nullptr, u_n, u_out, acc, static_cast<cudaStream_t>(cuda_stream));
+  // aliasing: two states are either the same buffer (where the stage table allows it) or disjoint ranges
+  const long long ext = state_extent(p, npatch);
+  if (stage == 1 && u_n != u_in) return SACRA_ERR_BADARG;           // stage 1 takes u_n from the stage input
+  if (overlap(u_out, ext, u_in, ext)) return SACRA_ERR_BADARG;      // u_in is read through the stencil
+  if (overlap(acc, ext, u_in, ext) || overlap(acc, ext, u_n, ext) || overlap(acc, ext, u_out, ext))
+    return SACRA_ERR_BADARG;
+  if (u_n != u_in && overlap(u_n, ext, u_in, ext)) return SACRA_ERR_BADARG;
+  if (u_n != u_out && overlap(u_n, ext, u_out, ext)) return SACRA_ERR_BADARG;
+  const int epi = (stage == 4 && (prm->flags & SACRA_FLAG_SKIP_INCREMENT)) ? 5 : stage;
+  return launch_z4c(p, npatch, prm, epi, u_in, nullptr, u_n, u_out, acc, static_cast<cudaStream_t>(cuda_stream));
 }
 
 int sacra_rk4_step(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, double* u, double* work,
@@ -634,7 +694,9 @@ int sacra_rk4_step(const sacra_patch_t* p, int npatch, const sacra_params_t* prm
       return SACRA_ERR_BADARG;   // the patch would run past the end of a state
   }
   if (!aligned16(u) || !aligned16(work)) return SACRA_ERR_ALIGN;
+  if (overlap(u, state_doubles, work, 3 * state_doubles)) return SACRA_ERR_BADARG;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int last = (prm->flags & SACRA_FLAG_SKIP_INCREMENT) ? 5 : 4;
   double* w0 = work;
   double* w1 = work + state_doubles;
   double* acc = work + 2 * state_doubles;
@@ -648,7 +710,7 @@ int sacra_rk4_step(const sacra_patch_t* p, int npatch, const sacra_params_t* prm
   if ((e = launch_fill(p, npatch, w1, st))) return e;
   if ((e = launch_z4c(p, npatch, prm, 3, w1, nullptr, u, w0, acc, st))) return e;
   if ((e = launch_fill(p, npatch, w0, st))) return e;
-  if ((e = launch_z4c(p, npatch, prm, 4, w0, nullptr, u, u, acc, st))) return e;
+  if ((e = launch_z4c(p, npatch, prm, last, w0, nullptr, u, u, acc, st))) return e;
   return launch_fill(p, npatch, u, st);
 }
 
@@ -656,8 +718,8 @@ int sacra_constraints(const sacra_patch_t* p, int npatch, const double* u, doubl
   if (!p || !u || !con) return SACRA_ERR_NULL;
   if (int e = check_patches(p, npatch)) return e;
   if (!aligned16(u) || !aligned16(con)) return SACRA_ERR_ALIGN;
-  if (u == con) return SACRA_ERR_BADARG;
-  const sacra_params_t none = {0.0, 0.0, 0.0, 0.0, 0.0, 1, 0};
+  if (overlap(u, state_extent(p, npatch), con, state_extent(p, npatch))) return SACRA_ERR_BADARG;
+  const sacra_params_t none = {0.0, 0.0, 0.0, 0.0, 0.0, 1, 0};   // the constraints have no parameters
   return launch_z4c(p, npatch, &none, -1, u, con, nullptr, nullptr, nullptr, static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -701,6 +763,7 @@ static int check_levels(const sacra_patch_t* parent, const sacra_patch_t* child,
   if (!parent || !child || !org) return SACRA_ERR_NULL;
   if (int e = check_patches(parent, 1)) return e;
   if (int e = check_patches(child, 1)) return e;
+  if (std::fabs(2.0 * child->dx - parent->dx) > 1e-12 * parent->dx) return SACRA_ERR_BADARG;   // 2:1 refinement
   const int nc[3] = {child->nx, child->ny, child->nz}, np[3] = {parent->nx, parent->ny, parent->nz};
   for (int a = 0; a < 3; ++a) {
     if (nc[a] & 1) return SACRA_ERR_BADARG;                                  // a parent cell holds two child cells
@@ -724,6 +787,7 @@ int sacra_restrict(const sacra_patch_t* parent, const sacra_patch_t* child, cons
   if (!u_parent || !u_child) return SACRA_ERR_NULL;
   if (int e = check_levels(parent, child, org, false)) return e;
   if (!aligned16(u_parent) || !aligned16(u_child)) return SACRA_ERR_ALIGN;
+  if (overlap(u_parent, state_extent(parent, 1), u_child, state_extent(child, 1))) return SACRA_ERR_BADARG;
   const LevelPair L = level_pair(parent, child, org);
   const int n = (child->nx / 2) * (child->ny / 2) * (child->nz / 2);
   k_restrict<<<dim3((n + 127) / 128, NF), 128, 0, static_cast<cudaStream_t>(cuda_stream)>>>(L, u_parent, u_child);
@@ -735,6 +799,7 @@ int sacra_prolong_ghosts(const sacra_patch_t* parent, const sacra_patch_t* child
   if (!u_parent || !u_child) return SACRA_ERR_NULL;
   if (int e = check_levels(parent, child, org, true)) return e;
   if (!aligned16(u_parent) || !aligned16(u_child)) return SACRA_ERR_ALIGN;
+  if (overlap(u_parent, state_extent(parent, 1), u_child, state_extent(child, 1))) return SACRA_ERR_BADARG;
   const LevelPair L = level_pair(parent, child, org);
   const int sx = child->nx + 2 * NG, sy = child->ny + 2 * NG;
   const int n = 2 * NG * (sx * sy + sx * child->nz + child->ny * child->nz);   // cells of the ghost shell
@@ -754,6 +819,6 @@ const char* sacra_strerror(int code) {
   }
 }
 
-const char* sacra_version(void) { return "0.1"; }
+const char* sacra_version(void) { return "0.2"; }
 
 }  // extern "C"

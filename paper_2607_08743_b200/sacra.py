@@ -17,6 +17,7 @@ from . import build as _build
 NF = 25
 NG = 3
 OK, ERR_NULL, ERR_BADARG, ERR_UNSUPPORTED, ERR_ALIGN, ERR_CUDA = 0, -1, -2, -3, -4, -5
+FLAG_SKIP_INCREMENT = 1
 EXPORTS = ("sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4_step",
            "sacra_strerror", "sacra_version",
            "sacra_constraints", "sacra_constraint_norms", "sacra_constraint_scratch_doubles",
@@ -34,7 +35,7 @@ class SacraParams(C.Structure):
     """sacra_params_t"""
     _fields_ = [("kappa1", C.c_double), ("kappa2", C.c_double), ("eta", C.c_double),
                 ("shift_coef", C.c_double), ("ko_sigma", C.c_double),
-                ("lapse_uses_khat", C.c_int32), ("reserved_", C.c_int32)]
+                ("lapse_uses_khat", C.c_int32), ("flags", C.c_int32)]
 
 
 class SacraError(RuntimeError):
@@ -94,7 +95,7 @@ def make_params(d):
     if isinstance(d, SacraParams):
         return d
     return SacraParams(d["kappa1"], d["kappa2"], d["eta"], d["shift_coef"], d["ko_sigma"],
-                       int(d.get("lapse_uses_khat", 1)), 0)
+                       int(d.get("lapse_uses_khat", 1)), int(d.get("flags", 0)))
 
 
 def _ptr(t):

@@ -123,3 +123,32 @@ def test_inter_level_argument_checks():
     assert _code(sacra.prolong_ghosts, pp[0], pc[0], (1, 4, 4), FAKE, FAKE + 64) == sacra.ERR_BADARG   # stencil leaves storage
     assert _code(sacra.prolong_ghosts, pp[0], pc[0], (4, 4, 11), FAKE, FAKE + 64) == sacra.ERR_BADARG
     assert _code(sacra.prolong_ghosts, pp[0], pc[0], ok, FAKE, None) == sacra.ERR_NULL
+
+
+def test_aliasing_is_checked_on_whole_states():
+    """two states are the same buffer where the stage table allows it, or disjoint ranges (sacra.h)"""
+    ps, total = _patch()
+    far = lambda k: FAKE + 8 * k * (total + 64)            # disjoint states
+    near = FAKE + 64                                       # inside the first state: a partial overlap
+    assert _code(sacra.z4c_rhs, ps, PRM, FAKE, near) == sacra.ERR_BADARG
+    assert _code(sacra.constraints, ps, FAKE, near) == sacra.ERR_BADARG
+    # stage 1 takes u_n from the stage input: u_n must be u_in
+    assert _code(sacra.rk4_substep, ps, PRM, 1, far(1), FAKE, far(2), far(3)) == sacra.ERR_BADARG
+    # partial overlaps of u_out / acc / u_n with anything
+    assert _code(sacra.rk4_substep, ps, PRM, 2, FAKE, far(1), far(1) + 64, far(3)) == sacra.ERR_BADARG
+    assert _code(sacra.rk4_substep, ps, PRM, 2, FAKE, far(1), far(2), far(2) + 64) == sacra.ERR_BADARG
+    assert _code(sacra.rk4_substep, ps, PRM, 2, FAKE, FAKE + 64, far(2), far(3)) == sacra.ERR_BADARG
+    assert _code(sacra.rk4_substep, ps, PRM, 3, FAKE, far(1), FAKE + 64, far(3)) == sacra.ERR_BADARG
+    # the work area of a step must not contain the state
+    assert _code(sacra.rk4_step, ps, PRM, FAKE + 8 * total, FAKE, total) == sacra.ERR_BADARG
+    assert _code(sacra.rk4_step, ps, PRM, FAKE, FAKE + 64, total) == sacra.ERR_BADARG
+
+
+def test_inter_level_spacing_and_overlap():
+    pp, tp = wl.make_layout([(16, 16, 16)], [0.2], [0.01], [(0, 0, 0)])
+    pc, _ = wl.make_layout([(8, 8, 8)], [0.1], [0.005], [(0, 0, 0)])
+    bad, _ = wl.make_layout([(8, 8, 8)], [0.2], [0.005], [(0, 0, 0)])
+    far = FAKE + 8 * (tp + 64)
+    assert _code(sacra.restrict, pp[0], bad[0], (4, 4, 4), FAKE, far) == sacra.ERR_BADARG       # not 2:1
+    assert _code(sacra.prolong_ghosts, pp[0], bad[0], (4, 4, 4), FAKE, far) == sacra.ERR_BADARG
+    assert _code(sacra.restrict, pp[0], pc[0], (4, 4, 4), FAKE, FAKE + 64) == sacra.ERR_BADARG   # states overlap
