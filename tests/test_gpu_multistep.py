@@ -126,3 +126,47 @@ def test_full_size_config4_all_points_against_oracle():
     chk = got.copy()
     orc.fill_ghosts(w.patches, chk)
     assert np.array_equal(chk, got)          # ghosts of the result are filled
+
+
+def test_repeatable_bit_for_bit_with_guard_bands():
+    """compute-sanitizer is closed on this GPU pool (profiles/r02_sanitizer.md), so races and stray accesses are looked
+    for directly: the state and the work area sit inside NaN guard bands (a read of a guard cell that reached a result
+    would poison it, a write would break the band), a ragged multi-patch batch is stepped 12 times from the same input
+    with other launches in between, and every run must give the same bits -- a race between the warps of a tile, between
+    a TMA refill and a late reader of a ring slot, or on the e arrays shows up as a changed bit."""
+    dims = [(37, 9, 11), (6, 6, 6), (16, 33, 7), (50, 13, 19)]
+    hs = [0.1, 0.15, 0.2, 0.12]
+    ps, total = wl.make_layout(dims, hs, [0.25 * h for h in hs], [(0.3, -0.2, 0.1)] * len(dims))
+    rng = np.random.default_rng(77)
+    w = wl.Workload("guard", ps, dict(wl.DEFAULT_PARAMS), np.zeros(total))
+    for ip, p in enumerate(ps):
+        for f in range(NF):
+            v = 0.02 * rng.normal(size=(p.nz, p.ny, p.nx))
+            if f in (wl.F_W, wl.F_G, wl.F_G + 3, wl.F_G + 5, wl.F_ALP):
+                v += 1.0
+            w.active_view(w.state, ip, f)[...] = v
+    G = 16384                                   # guard band, doubles (a multiple of 2: 16-byte alignment is kept)
+    big = torch.full((G + total + G + 3 * total + G,), float("nan"), dtype=torch.float64, device="cuda")
+    u, work = big[G:G + total], big[2 * G + total:2 * G + 4 * total]
+    first = None
+    other = dev(wl.make(0, n=16).state)
+    w0 = wl.make(0, n=16)
+    for rep in range(12):
+        u.copy_(torch.from_numpy(w.state))
+        work.zero_()
+        sacra.rk4_step(ps, w.params, u, work, total)
+        sacra.fill_ghosts(w0.patches, other)    # unrelated launches in between
+        res = (host(u).copy(), host(work[2 * total:]).copy())
+        assert np.all(np.isfinite(res[0]))
+        if first is None:
+            first = res
+        else:
+            assert np.array_equal(res[0], first[0]) and np.array_equal(res[1], first[1]), rep
+        bands = host(torch.cat([big[:G], big[G + total:2 * G + total], big[2 * G + 4 * total:]]))
+        assert np.all(np.isnan(bands)), rep
+    ref = w.state.copy()
+    S_ref = orc.rk4_step(ps, w.params, ref)
+    for ip in range(len(ps)):
+        for f in range(NF):
+            s = np.max(np.abs(w.active_view(S_ref, ip, f)))
+            assert np.max(np.abs(w.active_view(first[1], ip, f) - w.active_view(S_ref, ip, f))) <= RTOL * (s + FLOOR)
