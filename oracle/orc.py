@@ -175,3 +175,57 @@ def prolong_ghosts(parent, child, org, u_parent, u_child):
     lib().orc_prolong_ghosts(C.byref(_patches([parent])[0]), C.byref(_patches([child])[0]), o, _p(u_parent),
                              _p(u_child))
     return u_child
+
+
+# ---- physical boundaries: face modes 0 periodic, 1 mirror, 2 Sommerfeld, 3 none ---------------------
+BC_PERIODIC, BC_MIRROR, BC_SOMMERFELD, BC_NONE = 0, 1, 2, 3
+
+
+class OrcBoundary(C.Structure):
+    _fields_ = [("origin", C.c_double * 3), ("face", C.c_int32 * 6)]
+
+
+def _boundaries(bs):
+    """bs: list of (origin[3], face[6]) per patch"""
+    arr = (OrcBoundary * len(bs))()
+    for a, (o, f) in zip(arr, bs):
+        for i in range(3):
+            a.origin[i] = float(o[i])
+        for i in range(6):
+            a.face[i] = int(f[i])
+    return arr
+
+
+def fill_ghosts_faces(ps, bs, u):
+    lib().orc_fill_ghosts_faces(_patches(ps), _boundaries(bs), len(ps), _p(u))
+    return u
+
+
+def sommerfeld_rhs(ps, bs, u, rhs=None):
+    """Eq. 13 on the boundary shell (active cells within 3 cells of a Sommerfeld face); other cells of rhs untouched"""
+    if rhs is None:
+        rhs = np.zeros_like(u)
+    lib().orc_sommerfeld_rhs(_patches(ps), _boundaries(bs), len(ps), _p(u), _p(rhs))
+    return rhs
+
+
+def d1_bounded(u, i, lo, hi, h):
+    lib().orc_d1_bounded.restype = C.c_double
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    return lib().orc_d1_bounded(_p(u), int(i), int(lo), int(hi), C.c_double(h))
+
+
+def rk4_substep_bc(ps, bs, prm, stage, u_n, u_in, u_out, acc):
+    kbuf = np.zeros_like(u_in)
+    pr = _params(prm)
+    lib().orc_rk4_substep_bc(_patches(ps), _boundaries(bs), len(ps), C.byref(pr), int(stage), _p(u_n), _p(u_in),
+                             _p(u_out), _p(acc), _p(kbuf))
+
+
+def rk4_step_bc(ps, bs, prm, u):
+    """one RK4 step with per-face boundary modes, in place; returns the increment S per unit dt"""
+    pr = _params(prm)
+    n = u.size
+    work = np.zeros(4 * n)
+    lib().orc_rk4_step_bc(_patches(ps), _boundaries(bs), len(ps), C.byref(pr), _p(u), _p(work), C.c_int64(n))
+    return work[2 * n:3 * n].copy()

@@ -12,6 +12,7 @@
 #include <omp.h>
 #include "z4c_grid.hpp"
 #include "z4c_amr.hpp"
+#include "z4c_boundary.hpp"
 
 using namespace z4c_oracle;
 
@@ -159,6 +160,38 @@ void orc_count_ops(long* counts) {
   Cnt::add = Cnt::mul = Cnt::div = 0;
   derivs_at<Cnt>(f, 3 * sz + 3 * sy + 3, sy, sz, Cnt(0.1), Cnt(0.1), D);
   counts[3] = Cnt::add / NF; counts[4] = Cnt::mul / NF; counts[5] = Cnt::div / NF;
+}
+
+// ---- physical boundaries: per-face ghost fill, Sommerfeld shell, RK4 step with boundaries ----------
+struct orc_boundary { double origin[3]; int32_t face[6]; };
+static Boundary to_boundary(const orc_boundary& q) {
+  Boundary b;
+  for (int a = 0; a < 3; ++a) b.origin[a] = q.origin[a];
+  for (int a = 0; a < 6; ++a) b.face[a] = q.face[a];
+  return b;
+}
+void orc_fill_ghosts_faces(const orc_patch* ps, const orc_boundary* bs, int np, double* u) {
+  for (int q = 0; q < np; ++q) { Boundary b = to_boundary(bs[q]); fill_ghosts_faces<double>(to_patch(ps[q]), b.face, u); }
+}
+void orc_sommerfeld_rhs(const orc_patch* ps, const orc_boundary* bs, int np, const double* u, double* rhs) {
+  for (int q = 0; q < np; ++q) sommerfeld_rhs_patch<double>(to_patch(ps[q]), to_boundary(bs[q]), u, rhs);
+}
+// first derivative along x of a 1-D array of n samples at index i using indices lo..hi only (stencil pins)
+double orc_d1_bounded(const double* u, int i, int lo, int hi, double h) {
+  return d1_bounded<double>([&](int q) { return u[i + q]; }, i, lo, hi, 1.0 / (12.0 * h));
+}
+void orc_rk4_substep_bc(const orc_patch* ps, const orc_boundary* bs, int np, const orc_params* prm, int stage,
+                        const double* u_n, const double* u_in, double* u_out, double* acc, double* kbuf) {
+  auto P = to_params<double>(*prm);
+  for (int q = 0; q < np; ++q)
+    rk4_substep_bc<double>(to_patch(ps[q]), P, to_boundary(bs[q]), stage, u_n, u_in, u_out, acc, kbuf);
+}
+void orc_rk4_step_bc(const orc_patch* ps, const orc_boundary* bs, int np, const orc_params* prm, double* u,
+                     double* work, int64_t nstate) {
+  auto P = to_params<double>(*prm);
+  std::vector<Patch> v; std::vector<Boundary> b;
+  for (int q = 0; q < np; ++q) { v.push_back(to_patch(ps[q])); b.push_back(to_boundary(bs[q])); }
+  rk4_step_bc<double>(v.data(), b.data(), np, P, u, work, work + nstate, work + 2 * nstate, work + 3 * nstate);
 }
 
 // ---- __float128 referee ------------------------------------------------------
