@@ -94,6 +94,44 @@ int sacra_fill_ghosts(const sacra_patch_t* p, int npatch, double* u, void* cuda_
 #define SACRA_BC_MIRROR 1
 int sacra_fill_ghosts_bc(const sacra_patch_t* p, int npatch, const int32_t* axis_mode, double* u, void* cuda_stream);
 
+/* Physical boundaries per patch and face (section 2.2.2).
+ * face[] order: x- x+ y- y+ z- z+. Modes: SACRA_BC_PERIODIC and SACRA_BC_MIRROR as above (PERIODIC on both faces of an
+ * axis or on neither); SACRA_BC_SOMMERFELD: outer boundary with the outgoing-wave condition Eq. 13;
+ * SACRA_BC_NONE: the ghost cells behind the face belong to somebody else (e.g. sacra_prolong_ghosts) and are left alone.
+ * origin: coordinates of the centre of active cell (0,0,0); active cell (i,j,k) sits at origin + (i,j,k) dx (Eq. 13
+ * needs x^i / r; the origin of the coordinates must not be a cell of a boundary shell).
+ * Reading of Eq. 13 (the paper gives no discretisation): on the BOUNDARY SHELL -- the active cells
+ * within 3 cells of a SOMMERFELD face -- the right-hand side of all 25 fields is
+ *     d_t Q = -( x^i d_i Q + Q ) / r,   Q = field - flat value (1 for W, gt_xx, gt_yy, gt_zz, alpha; 0 otherwise),
+ * with 4th-order differences that use existing cells only: centred (-1 8 0 -8 1)/12h where it fits, else the lopsided
+ * (-3 -10 18 -6 1)/12h, else the one-sided (-25 48 -36 16 -3)/12h stencil pointing inwards; no KO term. Everywhere else
+ * the Z4c right-hand side applies (its stencils reach 3 cells, so it never reads a ghost cell behind a SOMMERFELD face;
+ * those ghost cells are neither read for a kept result nor written). */
+#define SACRA_BC_SOMMERFELD 2
+#define SACRA_BC_NONE 3
+typedef struct {
+  double origin[3];
+  int32_t face[6];
+} sacra_boundary_t;
+
+/* Halo fill with a mode per patch and face (bnd: HOST array of npatch entries). A ghost cell takes the active cell
+ * obtained by wrapping / reflecting every axis along which it lies outside; if one of those faces is SOMMERFELD or
+ * NONE the cell is left alone. */
+int sacra_fill_ghosts_faces(const sacra_patch_t* p, int npatch, const sacra_boundary_t* bnd, double* u, void* cuda_stream);
+
+/* Eq. 13 on the boundary shells: rhs receives the 25 Sommerfeld right-hand sides on the shell cells of every patch;
+ * all other cells of rhs are not touched. u: ghosts behind non-SOMMERFELD faces filled. rhs must not overlap u. */
+int sacra_sommerfeld_rhs(const sacra_patch_t* p, int npatch, const sacra_boundary_t* bnd, const double* u, double* rhs,
+                         void* cuda_stream);
+
+/* sacra_rk4_substep / sacra_rk4_step with physical boundaries: k is the Z4c right-hand side outside the boundary shells
+ * and Eq. 13 inside them (two kernels per substage: the fused substage kernel skips the shell cells, a small kernel
+ * applies the same stage table there); the halo fills of the step use the face modes. Same argument rules. */
+int sacra_rk4_substep_bc(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, const sacra_boundary_t* bnd,
+                         int stage, const double* u_n, const double* u_in, double* u_out, double* acc, void* cuda_stream);
+int sacra_rk4_step_bc(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, const sacra_boundary_t* bnd, double* u,
+                      double* work, int64_t state_doubles, void* cuda_stream);
+
 /* Z4c right-hand side including KO dissipation, F(u) (PAPER.md:49-73,
  * PAPER.md:99). u: ghosts already filled (read only). rhs: the 25 RHS values are written on active cells;
  * ghost cells and padding of rhs are not touched. rhs must not alias u. */

@@ -25,6 +25,7 @@ struct DevPatch {
   long long pitch, sz;     // doubles per x-row, doubles per z-plane
   long long fstride, offset;
   double dx, dt;
+  unsigned shell;          // bit 2a + side: that face is a Sommerfeld face (its 3 outermost layers are the boundary shell)
 };
 struct PatchBatch {
   DevPatch p[MAXP];
@@ -38,8 +39,14 @@ struct PatchBatch {
 // Only ghost cells are written and only active cells are read (every source index is mapped into the active range),
 // so reads and writes never overlap.
 // ---------------------------------------------------------------------------------------------------
-struct FillMode {
-  int m[3];   // per axis: 0 periodic, 1 mirror
+struct RkArgs {   // RK4 inputs / outputs of a substage (stage table of item 11)
+  const double* u_n;
+  double* u_out;
+  double* acc;
+};
+
+struct FillModes {
+  unsigned char m[MAXP][6];   // per patch and face (x- x+ y- y+ z- z+): 0 periodic, 1 mirror, 2 Sommerfeld, 3 none
 };
 // -1 for the a-component of a vector and for tensor components with exactly one index a
 __device__ __forceinline__ double field_parity(int f, int axis) {
@@ -54,40 +61,51 @@ __device__ __forceinline__ double field_parity(int f, int axis) {
   const int one[3] = {0b000110, 0b010010, 0b010100};   // x: xy xz | y: xy yz | z: xz yz
   return (one[axis] >> n) & 1 ? -1.0 : 1.0;
 }
-// storage index of the source cell of storage index I along an axis with n active cells; *refl: a mirror was used
-__device__ __forceinline__ int fill_source(int I, int n, int mode, bool* refl) {
+// storage index of the source cell of storage index I along an axis with n active cells and face modes lo / hi;
+// *refl: a mirror was used; *skip: the cell lies behind a face whose ghosts are not ours to fill (Sommerfeld, none)
+__device__ __forceinline__ int fill_source(int I, int n, int lo, int hi, bool* refl, bool* skip) {
   const int i = I - NG;
   *refl = false;
   if (i >= 0 && i < n) return I;
+  const int mode = i < 0 ? lo : hi;
+  if (mode >= 2) {
+    *skip = true;
+    return I;
+  }
   if (mode == 0) return (i < 0 ? i + n : i - n) + NG;
   *refl = true;
   return (i < 0 ? -1 - i : 2 * n - 1 - i) + NG;
 }
 
-__global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ PatchBatch B, const __grid_constant__ FillMode mode,
+__global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ PatchBatch B, const __grid_constant__ FillModes modes,
                                                      double* __restrict__ u) {
   int ip = 0;
 #pragma unroll 1
   while (ip + 1 < B.np && (int)blockIdx.x >= B.first_block[ip + 1]) ++ip;
   const DevPatch& p = B.p[ip];
+  const unsigned char* m = modes.m[ip];
   const int sx = p.nx + 2 * NG, sy = p.ny + 2 * NG;
   // one block = one storage plane K of one field: a ghost plane is copied whole, an active plane only
   // has its 6 ghost rows and the 3+3 x-ghosts of its active rows
   const int f = blockIdx.y;
   const int Kk = (int)blockIdx.x - B.first_block[ip];
-  bool rz, ry, rx;
-  const int Ks = fill_source(Kk, p.nz, mode.m[2], &rz);
+  bool rz, ry, rx, skz = false;
+  const int Ks = fill_source(Kk, p.nz, m[4], m[5], &rz, &skz);
+  if (skz) return;
   const bool plane_ghost = Ks != Kk;
   const double pz = rz ? field_parity(f, 2) : 1.0, py = field_parity(f, 1), px = field_parity(f, 0);
   double* fld = u + p.offset + (long long)f * p.fstride;
   double* dst = fld + (long long)Kk * p.sz;
   const double* src = fld + (long long)Ks * p.sz;
   auto copy_row = [&](int J) {   // one warp: the whole storage row J of this plane
-    const int Js = fill_source(J, p.ny, mode.m[1], &ry);
+    bool sky = false;
+    const int Js = fill_source(J, p.ny, m[2], m[3], &ry, &sky);
+    if (sky) return;
     const double s = pz * (ry ? py : 1.0);
     for (int I = threadIdx.x % 32; I < sx; I += 32) {
-      const int Is = fill_source(I, p.nx, mode.m[0], &rx);
-      dst[(long long)J * p.pitch + I] = (rx ? s * px : s) * src[(long long)Js * p.pitch + Is];
+      bool skx = false;
+      const int Is = fill_source(I, p.nx, m[0], m[1], &rx, &skx);
+      if (!skx) dst[(long long)J * p.pitch + I] = (rx ? s * px : s) * src[(long long)Js * p.pitch + Is];
     }
   };
   // blockIdx.z splits the work of a plane: a whole ghost plane copied by one block is a chain of ~300 dependent
@@ -100,9 +118,89 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
     for (int q = threadIdx.x + blockDim.x * blockIdx.z; q < p.ny * 2 * NG; q += blockDim.x * gridDim.z) {   // x-ghosts
       const int J = q / (2 * NG) + NG, c = q % (2 * NG);
       const int I = c < NG ? c : p.nx + c;
-      const int Is = fill_source(I, p.nx, mode.m[0], &rx);
-      dst[(long long)J * p.pitch + I] = (rx ? px : 1.0) * src[(long long)J * p.pitch + Is];
+      bool skx = false;
+      const int Is = fill_source(I, p.nx, m[0], m[1], &rx, &skx);
+      if (!skx) dst[(long long)J * p.pitch + I] = (rx ? px : 1.0) * src[(long long)J * p.pitch + Is];
     }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Sommerfeld boundary shell (Eq. 13): on the active cells within NG cells of a
+// Sommerfeld face the right-hand side of every field is  -( x^i d_i Q / r + Q / r ),  Q = u - flat value, with 4th-order
+// differences that use existing cells only (centred / lopsided / one-sided). Same operation order as the oracle
+// (oracle-independent restatement of DESIGN.md section 5.4; the library is built without FMA contraction): bit-identical.
+// EPI as in the substage kernel: 0 stores the RHS, 1..5 apply the RK4 stage table to the shell cells.
+// One block per active z-plane and field; threads walk the plane and skip the cells outside the shell.
+// ---------------------------------------------------------------------------------------------------
+struct ShellGeom {
+  double origin[MAXP][3];
+};
+__device__ __forceinline__ bool in_shell(const DevPatch& p, int i, int j, int k) {
+  const unsigned s = p.shell;
+  return ((s & 1u) && i < NG) || ((s & 2u) && i >= p.nx - NG) || ((s & 4u) && j < NG) || ((s & 8u) && j >= p.ny - NG) ||
+         ((s & 16u) && k < NG) || ((s & 32u) && k >= p.nz - NG);
+}
+// first derivative along a stride at index i of an axis whose usable index range is [lo, hi]
+__device__ __forceinline__ double d1_bounded(const double* u, long long st, int i, int lo, int hi, double inv12h) {
+  if (i - 2 >= lo && i + 2 <= hi) return (8.0 * (u[st] - u[-st]) - (u[2 * st] - u[-2 * st])) * inv12h;
+  const int s = (i - 2 < lo) ? 1 : -1;
+  const long long t = s * st;
+  const double u0 = u[0];
+  if (i - s >= lo && i - s <= hi)
+    return (double)s * ((((18.0 * (u[t] - u0) - 3.0 * (u[-t] - u0)) - 6.0 * (u[2 * t] - u0)) + (u[3 * t] - u0)) * inv12h);
+  return (double)s * ((((48.0 * (u[t] - u0) - 36.0 * (u[2 * t] - u0)) + 16.0 * (u[3 * t] - u0)) - 3.0 * (u[4 * t] - u0)) * inv12h);
+}
+template <int EPI>
+__global__ void __launch_bounds__(256) k_sommerfeld(const __grid_constant__ PatchBatch B, const __grid_constant__ ShellGeom G,
+                                                    const double* __restrict__ u_in, double* __restrict__ rhs,
+                                                    const __grid_constant__ RkArgs rk) {
+  int ip = 0;
+#pragma unroll 1
+  while (ip + 1 < B.np && (int)blockIdx.x >= B.first_block[ip + 1]) ++ip;
+  const DevPatch& p = B.p[ip];
+  if (!p.shell) return;
+  const int k = (int)blockIdx.x - B.first_block[ip], f = blockIdx.y;
+  const double h = p.dx, inv12h = 1.0 / (12.0 * h);
+  const int lo[3] = {(p.shell & 1u) ? 0 : -NG, (p.shell & 4u) ? 0 : -NG, (p.shell & 16u) ? 0 : -NG};
+  const int hi[3] = {(p.shell & 2u) ? p.nx - 1 : p.nx - 1 + NG, (p.shell & 8u) ? p.ny - 1 : p.ny - 1 + NG,
+                     (p.shell & 32u) ? p.nz - 1 : p.nz - 1 + NG};
+  const bool flat1 = f == F_W || f == F_G || f == F_G + 3 || f == F_G + 5 || f == F_ALP;
+  const long long fo = p.offset + (long long)f * p.fstride;
+  const double z = G.origin[ip][2] + (double)k * h;
+  for (int q = threadIdx.x; q < p.nx * p.ny; q += blockDim.x) {
+    const int i = q % p.nx, j = q / p.nx;
+    if (!in_shell(p, i, j, k)) continue;
+    const long long c = fo + (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
+    const double* uc = u_in + c;
+    const double x = G.origin[ip][0] + (double)i * h, y = G.origin[ip][1] + (double)j * h;
+    const double dx_ = d1_bounded(uc, 1, i, lo[0], hi[0], inv12h);
+    const double dy_ = d1_bounded(uc, p.pitch, j, lo[1], hi[1], inv12h);
+    const double dz_ = d1_bounded(uc, p.sz, k, lo[2], hi[2], inv12h);
+    const double r = sqrt((x * x + y * y) + z * z);
+    const double Q = uc[0] - (flat1 ? 1.0 : 0.0);
+    const double kk = -((((x * dx_ + y * dy_) + z * dz_) / r) + Q / r);
+    if (EPI == 0) {
+      rhs[c] = kk;
+      continue;
+    }
+    const double un = rk.u_n[c], dt = p.dt;
+    double acc_new, u_new;
+    if (EPI == 1) {
+      acc_new = kk;
+      u_new = un + (dt / 2.0) * kk;
+    } else if (EPI == 2) {
+      acc_new = rk.acc[c] + 2.0 * kk;
+      u_new = un + (dt / 2.0) * kk;
+    } else if (EPI == 3) {
+      acc_new = rk.acc[c] + 2.0 * kk;
+      u_new = un + dt * kk;
+    } else {
+      acc_new = (rk.acc[c] + kk) * (1.0 / 6.0);
+      u_new = un + dt * acc_new;
+    }
+    if (EPI != 5) rk.acc[c] = acc_new;
+    rk.u_out[c] = u_new;
   }
 }
 
@@ -119,11 +217,6 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
 using Tile = TileCfg<SACRA_TX, SACRA_TY, SACRA_TZ, SACRA_NS>;
 
 // EPI: 0 = store RHS; 1..4 = RK4 substage (item 11 table); 5 = substage 4 without the store of the increment S
-struct RkArgs {
-  const double* u_n;
-  double* u_out;
-  double* acc;
-};
 __host__ __device__ constexpr int rk_mode(int epi) { return epi == 0 ? 0 : (epi == 1 ? 1 : 2); }
 
 // Consumes the finished RHS values. The RK4 inputs never come from global loads: at stage 1 u_n is the stage
@@ -266,7 +359,8 @@ __global__ void __launch_bounds__(Tile::NTH, 1) k_z4c(const __grid_constant__ Pa
       src.has_next = tn < ntiles;
       src.iter = iter;
       const int i = id.bx * C::TX + tx, j = id.by * C::TY + ty, k = id.bz * C::TZ + tz;
-      const bool active = (i < p.nx) & (j < p.ny) & (k < p.nz);
+      // cells of the Sommerfeld boundary shell belong to k_sommerfeld
+      const bool active = (i < p.nx) & (j < p.ny) & (k < p.nz) && !(p.shell && in_shell(p, i, j, k));
       const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
       Emitter<(EPI < 0 ? 0 : EPI), Src> emit{src, rhs, rk.u_out, rk.acc, p.offset + c, p.fstride, p.dt, active};
       src.begin_tile();
@@ -469,6 +563,7 @@ static DevPatch to_dev(const sacra_patch_t& a) {
   d.nx = a.nx; d.ny = a.ny; d.nz = a.nz;
   d.pitch = a.pitch_x; d.sz = a.pitch_x * (long long)(a.ny + 2 * NG);
   d.fstride = a.field_stride; d.offset = a.patch_offset; d.dx = a.dx; d.dt = a.dt;
+  d.shell = 0;
   return d;
 }
 
@@ -479,14 +574,18 @@ static Params to_dev(const sacra_params_t& a) {
   return P;
 }
 
-static int launch_fill(const sacra_patch_t* p, int npatch, double* u, cudaStream_t st,
-                       FillMode mode = FillMode{{0, 0, 0}}) {
+// face modes of every patch: `axis_mode` (one mode per axis, both faces, every patch) or `bnd` (per patch and face)
+static int launch_fill(const sacra_patch_t* p, int npatch, double* u, cudaStream_t st, const int32_t* axis_mode = nullptr,
+                       const sacra_boundary_t* bnd = nullptr) {
   for (int q0 = 0; q0 < npatch; q0 += MAXP) {
     PatchBatch B;
+    FillModes M;
     B.np = (npatch - q0 < MAXP) ? npatch - q0 : MAXP;
     int nb = 0, split = 1;
     for (int q = 0; q < B.np; ++q) {
       B.p[q] = to_dev(p[q0 + q]);
+      for (int a = 0; a < 6; ++a)
+        M.m[q][a] = (unsigned char)(bnd ? bnd[q0 + q].face[a] : (axis_mode ? axis_mode[a / 2] : SACRA_BC_PERIODIC));
       B.first_block[q] = nb;
       nb += p[q0 + q].nz + 2 * NG;
       const long long plane = (long long)(p[q0 + q].nx + 2 * NG) * (p[q0 + q].ny + 2 * NG);
@@ -494,7 +593,61 @@ static int launch_fill(const sacra_patch_t* p, int npatch, double* u, cudaStream
       if (want > split) split = want;   // blocks per plane: only big planes are worth splitting
     }
     B.first_block[B.np] = nb;
-    k_fill_ghosts<<<dim3(nb, NF, split), 256, 0, st>>>(B, mode, u);
+    k_fill_ghosts<<<dim3(nb, NF, split), 256, 0, st>>>(B, M, u);
+    if (cudaGetLastError() != cudaSuccess) return SACRA_ERR_CUDA;
+  }
+  return SACRA_OK;
+}
+
+static int check_boundaries(const sacra_boundary_t* bnd, int npatch) {
+  if (!bnd) return SACRA_ERR_NULL;
+  for (int q = 0; q < npatch; ++q) {
+    for (int a = 0; a < 6; ++a)
+      if (bnd[q].face[a] < SACRA_BC_PERIODIC || bnd[q].face[a] > SACRA_BC_NONE) return SACRA_ERR_BADARG;
+    for (int a = 0; a < 3; ++a) {
+      if (!std::isfinite(bnd[q].origin[a])) return SACRA_ERR_BADARG;
+      // a periodic axis is periodic on both faces
+      if ((bnd[q].face[2 * a] == SACRA_BC_PERIODIC) != (bnd[q].face[2 * a + 1] == SACRA_BC_PERIODIC)) return SACRA_ERR_BADARG;
+    }
+  }
+  return SACRA_OK;
+}
+static unsigned shell_bits(const sacra_boundary_t& b) {
+  unsigned s = 0;
+  for (int a = 0; a < 6; ++a)
+    if (b.face[a] == SACRA_BC_SOMMERFELD) s |= 1u << a;
+  return s;
+}
+
+// Sommerfeld shell of every patch that has one: EPI 0 stores the RHS into `rhs`, 1..5 apply the RK4 stage table
+static int launch_sommerfeld(const sacra_patch_t* p, int npatch, const sacra_boundary_t* bnd, int epi, const double* u_in,
+                             double* rhs, const double* u_n, double* u_out, double* acc, cudaStream_t st) {
+  RkArgs rk{u_n, u_out, acc};
+  for (int q0 = 0; q0 < npatch; q0 += MAXP) {
+    PatchBatch B;
+    ShellGeom G;
+    B.np = (npatch - q0 < MAXP) ? npatch - q0 : MAXP;
+    int nb = 0;
+    bool any = false;
+    for (int q = 0; q < B.np; ++q) {
+      B.p[q] = to_dev(p[q0 + q]);
+      B.p[q].shell = shell_bits(bnd[q0 + q]);
+      any = any || B.p[q].shell;
+      for (int a = 0; a < 3; ++a) G.origin[q][a] = bnd[q0 + q].origin[a];
+      B.first_block[q] = nb;
+      nb += p[q0 + q].nz;
+    }
+    B.first_block[B.np] = nb;
+    if (!any) continue;
+    const dim3 grid(nb, NF);
+    switch (epi) {
+      case 0: k_sommerfeld<0><<<grid, 256, 0, st>>>(B, G, u_in, rhs, rk); break;
+      case 1: k_sommerfeld<1><<<grid, 256, 0, st>>>(B, G, u_in, rhs, rk); break;
+      case 2: k_sommerfeld<2><<<grid, 256, 0, st>>>(B, G, u_in, rhs, rk); break;
+      case 3: k_sommerfeld<3><<<grid, 256, 0, st>>>(B, G, u_in, rhs, rk); break;
+      case 4: k_sommerfeld<4><<<grid, 256, 0, st>>>(B, G, u_in, rhs, rk); break;
+      default: k_sommerfeld<5><<<grid, 256, 0, st>>>(B, G, u_in, rhs, rk); break;
+    }
     if (cudaGetLastError() != cudaSuccess) return SACRA_ERR_CUDA;
   }
   return SACRA_OK;
@@ -591,7 +744,7 @@ static cudaError_t launch_one(int grid, cudaStream_t st, const PatchBatch& B, co
 
 static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, int epi,
                       const double* u_in, double* rhs, const double* u_n, double* u_out, double* acc,
-                      cudaStream_t st) {
+                      cudaStream_t st, const sacra_boundary_t* bnd = nullptr) {
   const Params P = to_dev(*prm);
   RkArgs rk{u_n, u_out, acc};
   const int sms = num_sms();
@@ -604,6 +757,7 @@ static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* 
     for (int q = 0; q < B.np; ++q) {
       const sacra_patch_t& a = p[q0 + q];
       B.p[q] = to_dev(a);
+      if (bnd) B.p[q].shell = shell_bits(bnd[q0 + q]);
       B.first_block[q] = nb;
       nb += ((a.nx + Tile::TX - 1) / Tile::TX) * ((a.ny + Tile::TY - 1) / Tile::TY) * ((a.nz + Tile::TZ - 1) / Tile::TZ);
       if (int e = cached_map(a, u_in, Tile::PX, Tile::PY, Tile::PZ, 1, &M.box[q])) return e;
@@ -647,12 +801,9 @@ int sacra_fill_ghosts_bc(const sacra_patch_t* p, int npatch, const int32_t* axis
   if (!p || !u || !axis_mode) return SACRA_ERR_NULL;
   if (int e = check_patches(p, npatch)) return e;
   if (!aligned16(u)) return SACRA_ERR_ALIGN;
-  FillMode m;
-  for (int a = 0; a < 3; ++a) {
+  for (int a = 0; a < 3; ++a)
     if (axis_mode[a] != SACRA_BC_PERIODIC && axis_mode[a] != SACRA_BC_MIRROR) return SACRA_ERR_BADARG;
-    m.m[a] = axis_mode[a];
-  }
-  return launch_fill(p, npatch, u, static_cast<cudaStream_t>(cuda_stream), m);
+  return launch_fill(p, npatch, u, static_cast<cudaStream_t>(cuda_stream), axis_mode);
 }
 
 int sacra_z4c_rhs(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, const double* u, double* rhs,
@@ -712,6 +863,69 @@ int sacra_rk4_step(const sacra_patch_t* p, int npatch, const sacra_params_t* prm
   if ((e = launch_fill(p, npatch, w0, st))) return e;
   if ((e = launch_z4c(p, npatch, prm, last, w0, nullptr, u, u, acc, st))) return e;
   return launch_fill(p, npatch, u, st);
+}
+
+int sacra_fill_ghosts_faces(const sacra_patch_t* p, int npatch, const sacra_boundary_t* bnd, double* u, void* cuda_stream) {
+  if (!p || !u || !bnd) return SACRA_ERR_NULL;
+  if (int e = check_patches(p, npatch)) return e;
+  if (int e = check_boundaries(bnd, npatch)) return e;
+  if (!aligned16(u)) return SACRA_ERR_ALIGN;
+  return launch_fill(p, npatch, u, static_cast<cudaStream_t>(cuda_stream), nullptr, bnd);
+}
+
+int sacra_sommerfeld_rhs(const sacra_patch_t* p, int npatch, const sacra_boundary_t* bnd, const double* u, double* rhs,
+                         void* cuda_stream) {
+  if (!p || !u || !rhs || !bnd) return SACRA_ERR_NULL;
+  if (int e = check_patches(p, npatch)) return e;
+  if (int e = check_boundaries(bnd, npatch)) return e;
+  if (!aligned16(u) || !aligned16(rhs)) return SACRA_ERR_ALIGN;
+  const long long ext = state_extent(p, npatch);
+  if (overlap(u, ext, rhs, ext)) return SACRA_ERR_BADARG;
+  return launch_sommerfeld(p, npatch, bnd, 0, u, rhs, nullptr, nullptr, nullptr, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int sacra_rk4_substep_bc(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, const sacra_boundary_t* bnd,
+                         int stage, const double* u_n, const double* u_in, double* u_out, double* acc, void* cuda_stream) {
+  if (!p || !prm || !bnd || !u_n || !u_in || !u_out || !acc) return SACRA_ERR_NULL;
+  if (int e = check_patches(p, npatch)) return e;
+  if (int e = check_boundaries(bnd, npatch)) return e;
+  if (stage < 1 || stage > 4) return SACRA_ERR_BADARG;
+  if (!aligned16(u_n) || !aligned16(u_in) || !aligned16(u_out) || !aligned16(acc)) return SACRA_ERR_ALIGN;
+  const long long ext = state_extent(p, npatch);
+  if (stage == 1 && u_n != u_in) return SACRA_ERR_BADARG;
+  if (overlap(u_out, ext, u_in, ext)) return SACRA_ERR_BADARG;
+  if (overlap(acc, ext, u_in, ext) || overlap(acc, ext, u_n, ext) || overlap(acc, ext, u_out, ext)) return SACRA_ERR_BADARG;
+  if (u_n != u_in && overlap(u_n, ext, u_in, ext)) return SACRA_ERR_BADARG;
+  if (u_n != u_out && overlap(u_n, ext, u_out, ext)) return SACRA_ERR_BADARG;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int epi = (stage == 4 && (prm->flags & SACRA_FLAG_SKIP_INCREMENT)) ? 5 : stage;
+  if (int e = launch_z4c(p, npatch, prm, epi, u_in, nullptr, u_n, u_out, acc, st, bnd)) return e;
+  return launch_sommerfeld(p, npatch, bnd, epi, u_in, nullptr, u_n, u_out, acc, st);
+}
+
+int sacra_rk4_step_bc(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, const sacra_boundary_t* bnd, double* u,
+                      double* work, int64_t state_doubles, void* cuda_stream) {
+  if (!p || !prm || !bnd || !u || !work) return SACRA_ERR_NULL;
+  if (int e = check_patches(p, npatch)) return e;
+  if (int e = check_boundaries(bnd, npatch)) return e;
+  if (state_doubles < 1 || (state_doubles & 1) || state_extent(p, npatch) > state_doubles) return SACRA_ERR_BADARG;
+  if (!aligned16(u) || !aligned16(work)) return SACRA_ERR_ALIGN;
+  if (overlap(u, state_doubles, work, 3 * state_doubles)) return SACRA_ERR_BADARG;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int last = (prm->flags & SACRA_FLAG_SKIP_INCREMENT) ? 5 : 4;
+  double* w0 = work;
+  double* w1 = work + state_doubles;
+  double* acc = work + 2 * state_doubles;
+  const double* in[4] = {u, w0, w1, w0};
+  double* out[4] = {w0, w1, w0, u};
+  int e;
+  for (int s = 0; s < 4; ++s) {
+    if ((e = launch_fill(p, npatch, const_cast<double*>(in[s]), st, nullptr, bnd))) return e;
+    const int epi = s == 3 ? last : s + 1;
+    if ((e = launch_z4c(p, npatch, prm, epi, in[s], nullptr, u, out[s], acc, st, bnd))) return e;
+    if ((e = launch_sommerfeld(p, npatch, bnd, epi, in[s], nullptr, u, out[s], acc, st))) return e;
+  }
+  return launch_fill(p, npatch, u, st, nullptr, bnd);
 }
 
 int sacra_constraints(const sacra_patch_t* p, int npatch, const double* u, double* con, void* cuda_stream) {

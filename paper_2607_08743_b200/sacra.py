@@ -21,7 +21,8 @@ FLAG_SKIP_INCREMENT = 1
 EXPORTS = ("sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4_step",
            "sacra_strerror", "sacra_version",
            "sacra_constraints", "sacra_constraint_norms", "sacra_constraint_scratch_doubles",
-           "sacra_fill_ghosts_bc", "sacra_restrict", "sacra_prolong_ghosts")
+           "sacra_fill_ghosts_bc", "sacra_restrict", "sacra_prolong_ghosts",
+           "sacra_fill_ghosts_faces", "sacra_sommerfeld_rhs", "sacra_rk4_substep_bc", "sacra_rk4_step_bc")
 
 
 class SacraPatch(C.Structure):
@@ -36,6 +37,11 @@ class SacraParams(C.Structure):
     _fields_ = [("kappa1", C.c_double), ("kappa2", C.c_double), ("eta", C.c_double),
                 ("shift_coef", C.c_double), ("ko_sigma", C.c_double),
                 ("lapse_uses_khat", C.c_int32), ("flags", C.c_int32)]
+
+
+class SacraBoundary(C.Structure):
+    """sacra_boundary_t"""
+    _fields_ = [("origin", C.c_double * 3), ("face", C.c_int32 * 6)]
 
 
 class SacraError(RuntimeError):
@@ -60,7 +66,11 @@ def _load():
     lib.sacra_fill_ghosts_bc.argtypes = [vp, i32, vp, dp, vp]
     lib.sacra_restrict.argtypes = [vp, vp, vp, dp, dp, vp]
     lib.sacra_prolong_ghosts.argtypes = [vp, vp, vp, dp, dp, vp]
-    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:12]:
+    lib.sacra_fill_ghosts_faces.argtypes = [vp, i32, vp, dp, vp]
+    lib.sacra_sommerfeld_rhs.argtypes = [vp, i32, vp, dp, dp, vp]
+    lib.sacra_rk4_substep_bc.argtypes = [vp, i32, vp, vp, i32, dp, dp, dp, dp, vp]
+    lib.sacra_rk4_step_bc.argtypes = [vp, i32, vp, vp, dp, dp, i64, vp]
+    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:16]:
         getattr(lib, n).restype = C.c_int
     lib.sacra_strerror.argtypes = [C.c_int]
     lib.sacra_strerror.restype = C.c_char_p
@@ -172,7 +182,47 @@ def constraint_norms(patches, con, scratch, norms, stream=None):
                                       _stream(stream)))
 
 
-BC_PERIODIC, BC_MIRROR = 0, 1
+BC_PERIODIC, BC_MIRROR, BC_SOMMERFELD, BC_NONE = 0, 1, 2, 3
+
+
+def make_boundaries(bs):
+    """list of (origin[3], face[6]) per patch -> (SacraBoundary*n)"""
+    if bs is None or isinstance(bs, C.Array):
+        return bs
+    arr = (SacraBoundary * len(bs))()
+    for a, (o, f) in zip(arr, bs):
+        for i in range(3):
+            a.origin[i] = float(o[i])
+        for i in range(6):
+            a.face[i] = int(f[i])
+    return arr
+
+
+def fill_ghosts_faces(patches, bnd, u, stream=None):
+    ps = make_patches(patches) if patches is not None else None
+    _check(lib.sacra_fill_ghosts_faces(ps, len(ps) if ps is not None else 0, make_boundaries(bnd), _ptr(u), _stream(stream)))
+
+
+def sommerfeld_rhs(patches, bnd, u, rhs, stream=None):
+    ps = make_patches(patches) if patches is not None else None
+    _check(lib.sacra_sommerfeld_rhs(ps, len(ps) if ps is not None else 0, make_boundaries(bnd), _ptr(u), _ptr(rhs),
+                                    _stream(stream)))
+
+
+def rk4_substep_bc(patches, params, bnd, stage, u_n, u_in, u_out, acc, stream=None):
+    ps = make_patches(patches) if patches is not None else None
+    pr = make_params(params) if params is not None else None
+    _check(lib.sacra_rk4_substep_bc(ps, len(ps) if ps is not None else 0, _ref(pr), make_boundaries(bnd), int(stage),
+                                    _ptr(u_n), _ptr(u_in), _ptr(u_out), _ptr(acc), _stream(stream)))
+
+
+def rk4_step_bc(patches, params, bnd, u, work, state_doubles=None, stream=None):
+    ps = make_patches(patches) if patches is not None else None
+    pr = make_params(params) if params is not None else None
+    if state_doubles is None:
+        state_doubles = u.numel()
+    _check(lib.sacra_rk4_step_bc(ps, len(ps) if ps is not None else 0, _ref(pr), make_boundaries(bnd), _ptr(u), _ptr(work),
+                                 int(state_doubles), _stream(stream)))
 
 
 def fill_ghosts_bc(patches, axis_mode, u, stream=None):

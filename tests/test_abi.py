@@ -152,3 +152,20 @@ def test_inter_level_spacing_and_overlap():
     assert _code(sacra.restrict, pp[0], bad[0], (4, 4, 4), FAKE, far) == sacra.ERR_BADARG       # not 2:1
     assert _code(sacra.prolong_ghosts, pp[0], bad[0], (4, 4, 4), FAKE, far) == sacra.ERR_BADARG
     assert _code(sacra.restrict, pp[0], pc[0], (4, 4, 4), FAKE, FAKE + 64) == sacra.ERR_BADARG   # states overlap
+
+
+def test_boundary_argument_checks():
+    ps, total = _patch()
+    ok = [((1.0, 2.0, 3.0), [2, 2, 2, 2, 1, 2])]
+    far = FAKE + 8 * (total + 64)
+    assert C.sizeof(sacra.SacraBoundary) == 3 * 8 + 6 * 4
+    assert _code(sacra.fill_ghosts_faces, ps, None, FAKE) == sacra.ERR_NULL
+    assert _code(sacra.fill_ghosts_faces, ps, [((0, 0, 0), [0, 1, 2, 2, 2, 2])], FAKE) == sacra.ERR_BADARG   # half-periodic axis
+    assert _code(sacra.fill_ghosts_faces, ps, [((0, 0, 0), [4, 2, 2, 2, 2, 2])], FAKE) == sacra.ERR_BADARG   # unknown mode
+    assert _code(sacra.fill_ghosts_faces, ps, [((float("nan"), 0, 0), [2] * 6)], FAKE) == sacra.ERR_BADARG
+    assert _code(sacra.sommerfeld_rhs, ps, ok, FAKE, FAKE + 64) == sacra.ERR_BADARG                       # overlap
+    assert _code(sacra.sommerfeld_rhs, ps, ok, FAKE, far + 8) == sacra.ERR_ALIGN
+    assert _code(sacra.rk4_substep_bc, ps, PRM, ok, 1, far, FAKE, far + 8 * (total + 64), far + 16 * (total + 64)) == sacra.ERR_BADARG
+    assert _code(sacra.rk4_substep_bc, ps, PRM, ok, 7, FAKE, FAKE, far, far + 8 * (total + 64)) == sacra.ERR_BADARG
+    assert _code(sacra.rk4_step_bc, ps, PRM, ok, FAKE, FAKE + 64, total) == sacra.ERR_BADARG
+    assert _code(sacra.rk4_step_bc, ps, PRM, None, FAKE, far, total) == sacra.ERR_NULL

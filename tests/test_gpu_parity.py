@@ -175,7 +175,8 @@ def test_substep_stage_table_against_oracle():
         orc.rk4_substep(ps, prm, stage, un, uin, out_ref, acc_ref)
         out_gpu = torch.zeros_like(acc_gpu)
         acc_in = acc_ref.copy()
-        sacra.rk4_substep(ps, prm, stage, dev(un), dev(uin), out_gpu, acc_gpu)
+        d_un = dev(un)      # stage 1 takes u_n from the stage input: the same buffer
+        sacra.rk4_substep(ps, prm, stage, d_un, d_un if stage == 1 else dev(uin), out_gpu, acc_gpu)
         _assert_parity(w, host(acc_gpu), acc_ref, "acc stage %d" % stage)
         _assert_state(w, host(out_gpu), out_ref, k_ref)
         # next stage input: oracle's own (keeps the comparison stage-local)
@@ -191,7 +192,8 @@ def test_substep_leaves_ghosts_and_padding_untouched():
     for stage in (1, 4):
         out = torch.full((un.size,), float("nan"), dtype=torch.float64, device="cuda")
         acc = torch.full((un.size,), 0.5, dtype=torch.float64, device="cuda")
-        sacra.rk4_substep(ps, prm, stage, dev(un), dev(un), out, acc)
+        d_un = dev(un)
+        sacra.rk4_substep(ps, prm, stage, d_un, d_un, out, acc)
         assert _untouched_outside_active(w, host(out))
         acc_h, out_h = host(acc), host(out)
         for ip in range(len(ps)):
