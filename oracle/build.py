@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(HERE, "liborc_z4c.so")
 SRCS = ["z4c_oracle_capi.cpp"]
-DEPS = SRCS + ["z4c_oracle.hpp", "z4c_algebra.hpp", "z4c_grid.hpp", "z4c_amr.hpp", "z4c_boundary.hpp"]
+DEPS = SRCS + ["z4c_oracle.hpp", "z4c_algebra.hpp", "z4c_grid.hpp", "z4c_amr.hpp", "z4c_boundary.hpp", "z4c_subcycle.hpp"]
 FLAGS = ["-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
          "-shared", "-fPIC", "-Wall"]
 

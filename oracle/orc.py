@@ -229,3 +229,31 @@ def rk4_step_bc(ps, bs, prm, u):
     work = np.zeros(4 * n)
     lib().orc_rk4_step_bc(_patches(ps), _boundaries(bs), len(ps), C.byref(pr), _p(u), _p(work), C.c_int64(n))
     return work[2 * n:3 * n].copy()
+
+
+# ---- subcycling: time interpolation of the parent levels and one Berger-Oliger step of a pair ----------
+def time_weights(n, theta):
+    """weights of the parent time levels at theta = (t - t_n)/dt: n = 2 (U^n, U^n+1), n = 3 (U^n-1, U^n, U^n+1)"""
+    w = np.zeros(3)
+    lib().orc_time_weights(int(n), C.c_double(theta), _p(w))
+    return w
+
+
+def lincomb(p, levels, w):
+    """(w0 u0 + w1 u1) [+ w2 u2] on every storage cell of patch p"""
+    out = np.zeros_like(levels[0])
+    n = len(levels)
+    u = list(levels) + [levels[0]] * (3 - n)
+    lib().orc_lincomb(C.byref(_patches([p])[0]), n, _p(u[0]), _p(u[1]), _p(u[2]), _p(np.ascontiguousarray(w, dtype=np.float64)),
+                      _p(out))
+    return out
+
+
+def subcycle_step(parent, child, org, prm, bnd, u_parent, u_parent_prev, have_prev, u_child):
+    """one Berger-Oliger step of a parent / child pair, in place; bnd = (origin, faces) of the parent.
+    u_parent_prev: buffer that receives the parent state the step started from (read as U^n-1 if have_prev)."""
+    o = (C.c_int32 * 3)(*[int(v) for v in org])
+    pr = _params(prm)
+    lib().orc_subcycle_step(C.byref(_patches([parent])[0]), C.byref(_patches([child])[0]), o, C.byref(pr),
+                            C.byref(_boundaries([bnd])[0]), _p(u_parent), _p(u_parent_prev), int(bool(have_prev)),
+                            _p(u_child), C.c_int64(u_parent.size), C.c_int64(u_child.size))

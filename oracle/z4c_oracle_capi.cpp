@@ -13,6 +13,7 @@
 #include "z4c_grid.hpp"
 #include "z4c_amr.hpp"
 #include "z4c_boundary.hpp"
+#include "z4c_subcycle.hpp"
 
 using namespace z4c_oracle;
 
@@ -192,6 +193,21 @@ void orc_rk4_step_bc(const orc_patch* ps, const orc_boundary* bs, int np, const 
   std::vector<Patch> v; std::vector<Boundary> b;
   for (int q = 0; q < np; ++q) { v.push_back(to_patch(ps[q])); b.push_back(to_boundary(bs[q])); }
   rk4_step_bc<double>(v.data(), b.data(), np, P, u, work, work + nstate, work + 2 * nstate, work + 3 * nstate);
+}
+
+// ---- subcycling: time weights, linear combination of parent levels, one Berger-Oliger step ---------
+void orc_time_weights(int n, double theta, double* w) { time_weights<double>(n, theta, w); }
+void orc_lincomb(const orc_patch* p, int n, const double* u0, const double* u1, const double* u2, const double* w,
+                 double* out) {
+  const double* u[3] = {u0, u1, u2};
+  lincomb_patch<double>(to_patch(*p), n, u, w, out);
+}
+void orc_subcycle_step(const orc_patch* parent, const orc_patch* child, const int32_t* org, const orc_params* prm,
+                       const orc_boundary* bnd, double* u_parent, double* u_parent_prev, int have_prev, double* u_child,
+                       int64_t n_parent, int64_t n_child) {
+  const int o[3] = {org[0], org[1], org[2]};
+  subcycle_step<double>(to_patch(*parent), to_patch(*child), o, to_params<double>(*prm), to_boundary(*bnd), u_parent,
+                        u_parent_prev, have_prev != 0, u_child, n_parent, n_child);
 }
 
 // ---- __float128 referee ------------------------------------------------------
