@@ -198,6 +198,31 @@ int sacra_restrict(const sacra_patch_t* parent, const sacra_patch_t* child, cons
 int sacra_prolong_ghosts(const sacra_patch_t* parent, const sacra_patch_t* child, const int32_t* org,
                          const double* u_parent, double* u_child, void* cuda_stream);
 
+/* Time interpolation of the refinement-boundary data and the Berger-Oliger step of a parent / child pair (SURVEY 8(f)
+ * f-3; the child advances with a halved time step, two steps per parent step; its boundary data at the
+ * substeps "are interpolated between the parent time levels, at first order in the very first time step of a run and at
+ * second order thereafter"). theta = (t - t_n) / dt_parent.
+ *   sacra_time_weights   HOST function, no GPU work: weights of the parent time levels at theta. nlevels = 2: the line
+ *                        through U^n, U^n+1 (w[2] = 0); nlevels = 3: the parabola through U^n-1, U^n, U^n+1. w: HOST double[3].
+ *   sacra_lincomb        out = (w[0] u0 + w[1] u1) [+ w[2] u2] on every storage cell (ghosts included) of ONE patch, all
+ *                        25 fields; w: HOST double[3]; out must not overlap the inputs.
+ *   sacra_subcycle_step  one step of the pair: (1) the parent takes one RK4 step with its boundary modes
+ *                        (sacra_rk4_step_bc); (2) the child takes two RK4 steps of dt/2: before every substage the ghost
+ *                        cells of the stage input are prolonged (sacra_prolong_ghosts) from the parent levels
+ *                        interpolated to the substage time theta = (m + c_s)/2, m = 0, 1, c = (0, 1/2, 1/2, 1); (3) the
+ *                        child's ghosts are prolonged from the new parent state, the child is restricted onto the
+ *                        covered parent cells (sacra_restrict) and the parent's ghosts are refilled.
+ *                        u_parent_prev: on entry U^n-1 if have_prev != 0 (else ignored), on return U^n (the state the
+ *                        step started from). work_parent: 5 x parent_doubles, work_child: 3 x child_doubles doubles.
+ *                        child->dt must be parent->dt / 2; geometry rules as for sacra_prolong_ghosts. */
+int sacra_time_weights(int nlevels, double theta, double* w);
+int sacra_lincomb(const sacra_patch_t* p, int nlevels, const double* u0, const double* u1, const double* u2, const double* w,
+                  double* out, void* cuda_stream);
+int sacra_subcycle_step(const sacra_patch_t* parent, const sacra_patch_t* child, const int32_t* org,
+                        const sacra_params_t* prm, const sacra_boundary_t* parent_bnd, double* u_parent,
+                        double* u_parent_prev, int have_prev, double* u_child, double* work_parent,
+                        int64_t parent_doubles, double* work_child, int64_t child_doubles, void* cuda_stream);
+
 /* Static description of a status code (never NULL). */
 const char* sacra_strerror(int code);
 

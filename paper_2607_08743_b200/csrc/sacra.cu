@@ -520,6 +520,25 @@ __global__ void __launch_bounds__(128) k_prolong_ghosts(const __grid_constant__ 
   u_child[pc.offset + (long long)blockIdx.y * pc.fstride + (long long)Kk * pc.sz + (long long)J * pc.pitch + I] = az;
 }
 
+// linear combination of up to three states on every storage cell of a patch (time interpolation of the parent levels,
+// SURVEY 8(f) f-3): out = (w0 u0 + w1 u1) [+ w2 u2], one rounding per operation like the oracle's
+struct LinComb {
+  const double* u[3];
+  double w[3];
+  int n;
+};
+__global__ void __launch_bounds__(256) k_lincomb(const __grid_constant__ DevPatch p, const __grid_constant__ LinComb L,
+                                                 double* __restrict__ out) {
+  const int sx = p.nx + 2 * NG, sy = p.ny + 2 * NG;
+  const long long c0 = p.offset + (long long)blockIdx.y * p.fstride + (long long)blockIdx.x * p.sz;
+  for (int q = threadIdx.x; q < sx * sy; q += blockDim.x) {
+    const long long c = c0 + (long long)(q / sx) * p.pitch + (q % sx);
+    double s = L.w[0] * L.u[0][c] + L.w[1] * L.u[1][c];
+    if (L.n == 3) s = s + L.w[2] * L.u[2][c];
+    out[c] = s;
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------
 // Host side: validation and launches
 // ---------------------------------------------------------------------------------------------------
@@ -1019,6 +1038,103 @@ int sacra_prolong_ghosts(const sacra_patch_t* parent, const sacra_patch_t* child
   const int n = 2 * NG * (sx * sy + sx * child->nz + child->ny * child->nz);   // cells of the ghost shell
   k_prolong_ghosts<<<dim3((n + 127) / 128, NF), 128, 0, static_cast<cudaStream_t>(cuda_stream)>>>(L, u_parent, u_child);
   return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
+}
+
+int sacra_time_weights(int nlevels, double theta, double* w) {
+  if (!w) return SACRA_ERR_NULL;
+  if ((nlevels != 2 && nlevels != 3) || !std::isfinite(theta)) return SACRA_ERR_BADARG;
+  if (nlevels == 2) {            // straight line through theta = 0, 1
+    w[0] = 1.0 - theta; w[1] = theta; w[2] = 0.0;
+  } else {                       // parabola through theta = -1, 0, 1 (Lagrange basis)
+    w[0] = (theta * (theta - 1.0)) / 2.0;
+    w[1] = ((theta + 1.0) * (theta - 1.0)) / -1.0;
+    w[2] = ((theta + 1.0) * theta) / 2.0;
+  }
+  return SACRA_OK;
+}
+
+static int launch_lincomb(const sacra_patch_t* p, int n, const double* u0, const double* u1, const double* u2,
+                          const double* w, double* out, cudaStream_t st) {
+  LinComb L;
+  L.u[0] = u0; L.u[1] = u1; L.u[2] = n == 3 ? u2 : u0;
+  L.w[0] = w[0]; L.w[1] = w[1]; L.w[2] = n == 3 ? w[2] : 0.0;
+  L.n = n;
+  k_lincomb<<<dim3(p->nz + 2 * NG, NF), 256, 0, st>>>(to_dev(*p), L, out);
+  return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
+}
+
+int sacra_lincomb(const sacra_patch_t* p, int nlevels, const double* u0, const double* u1, const double* u2, const double* w,
+                  double* out, void* cuda_stream) {
+  if (!p || !u0 || !u1 || !w || !out || (nlevels == 3 && !u2)) return SACRA_ERR_NULL;
+  if (int e = check_patches(p, 1)) return e;
+  if (nlevels != 2 && nlevels != 3) return SACRA_ERR_BADARG;
+  if (!aligned16(u0) || !aligned16(u1) || !aligned16(out) || (nlevels == 3 && !aligned16(u2))) return SACRA_ERR_ALIGN;
+  const long long ext = state_extent(p, 1);
+  if (overlap(out, ext, u0, ext) || overlap(out, ext, u1, ext) || (nlevels == 3 && overlap(out, ext, u2, ext)))
+    return SACRA_ERR_BADARG;
+  return launch_lincomb(p, nlevels, u0, u1, u2, w, out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int sacra_subcycle_step(const sacra_patch_t* parent, const sacra_patch_t* child, const int32_t* org,
+                        const sacra_params_t* prm, const sacra_boundary_t* parent_bnd, double* u_parent,
+                        double* u_parent_prev, int have_prev, double* u_child, double* work_parent,
+                        int64_t parent_doubles, double* work_child, int64_t child_doubles, void* cuda_stream) {
+  if (!prm || !parent_bnd || !u_parent || !u_parent_prev || !u_child || !work_parent || !work_child) return SACRA_ERR_NULL;
+  if (int e = check_levels(parent, child, org, true)) return e;
+  if (int e = check_boundaries(parent_bnd, 1)) return e;
+  if (std::fabs(2.0 * child->dt - parent->dt) > 1e-12 * std::fabs(parent->dt)) return SACRA_ERR_BADARG;   // halved time step
+  if (parent_doubles < state_extent(parent, 1) || child_doubles < state_extent(child, 1) || (parent_doubles & 1) ||
+      (child_doubles & 1))
+    return SACRA_ERR_BADARG;
+  if (!aligned16(u_parent) || !aligned16(u_parent_prev) || !aligned16(u_child) || !aligned16(work_parent) ||
+      !aligned16(work_child))
+    return SACRA_ERR_ALIGN;
+  const double* bufs[5] = {u_parent, u_parent_prev, u_child, work_parent, work_child};
+  const long long len[5] = {parent_doubles, parent_doubles, child_doubles, 5 * parent_doubles, 3 * child_doubles};
+  for (int a = 0; a < 5; ++a)
+    for (int b = a + 1; b < 5; ++b)
+      if (overlap(bufs[a], len[a], bufs[b], len[b])) return SACRA_ERR_BADARG;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  double* old = work_parent;
+  double* tmp = work_parent + parent_doubles;
+  double* wk = work_parent + 2 * parent_doubles;
+  int e;
+  // (1) the parent: t_n -> t_n + dt
+  if (cudaMemcpyAsync(old, u_parent, (size_t)parent_doubles * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return SACRA_ERR_CUDA;
+  if ((e = sacra_rk4_step_bc(parent, 1, prm, parent_bnd, u_parent, wk, parent_doubles, cuda_stream))) return e;
+  // (2) the child: two steps of dt / 2, ghosts of every stage input from the parent levels interpolated in time
+  const int nlev = have_prev ? 3 : 2;
+  const double* lev[3] = {have_prev ? u_parent_prev : old, have_prev ? old : u_parent, have_prev ? u_parent : nullptr};
+  double* w0 = work_child;
+  double* w1 = work_child + child_doubles;
+  double* acc = work_child + 2 * child_doubles;
+  const double cs[4] = {0.0, 0.5, 0.5, 1.0};
+  const LevelPair L = level_pair(parent, child, org);
+  const int sx = child->nx + 2 * NG, sy = child->ny + 2 * NG;
+  const int nshell = 2 * NG * (sx * sy + sx * child->nz + child->ny * child->nz);
+  auto prolong = [&](const double* up, double* uc) {
+    k_prolong_ghosts<<<dim3((nshell + 127) / 128, NF), 128, 0, st>>>(L, up, uc);
+    return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
+  };
+  for (int m = 0; m < 2; ++m) {
+    const double* in[4] = {u_child, w0, w1, w0};
+    double* out[4] = {w0, w1, w0, u_child};
+    for (int s = 0; s < 4; ++s) {
+      double w[3];
+      sacra_time_weights(nlev, ((double)m + cs[s]) / 2.0, w);
+      if ((e = launch_lincomb(parent, nlev, lev[0], lev[1], lev[2], w, tmp, st))) return e;
+      if ((e = prolong(tmp, const_cast<double*>(in[s])))) return e;
+      if ((e = launch_z4c(child, 1, prm, s + 1, in[s], nullptr, u_child, out[s], acc, st))) return e;
+    }
+  }
+  // (3) child ghosts at the new time, restriction, parent ghosts; U^n goes to the caller for the next step
+  if ((e = prolong(u_parent, u_child))) return e;
+  const int nr = (child->nx / 2) * (child->ny / 2) * (child->nz / 2);
+  k_restrict<<<dim3((nr + 127) / 128, NF), 128, 0, st>>>(L, u_parent, u_child);
+  if (cudaGetLastError() != cudaSuccess) return SACRA_ERR_CUDA;
+  if ((e = launch_fill(parent, 1, u_parent, st, nullptr, parent_bnd))) return e;
+  if (cudaMemcpyAsync(u_parent_prev, old, (size_t)parent_doubles * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return SACRA_ERR_CUDA;
+  return SACRA_OK;
 }
 
 const char* sacra_strerror(int code) {

@@ -22,7 +22,8 @@ EXPORTS = ("sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4
            "sacra_strerror", "sacra_version",
            "sacra_constraints", "sacra_constraint_norms", "sacra_constraint_scratch_doubles",
            "sacra_fill_ghosts_bc", "sacra_restrict", "sacra_prolong_ghosts",
-           "sacra_fill_ghosts_faces", "sacra_sommerfeld_rhs", "sacra_rk4_substep_bc", "sacra_rk4_step_bc")
+           "sacra_fill_ghosts_faces", "sacra_sommerfeld_rhs", "sacra_rk4_substep_bc", "sacra_rk4_step_bc",
+           "sacra_time_weights", "sacra_lincomb", "sacra_subcycle_step")
 
 
 class SacraPatch(C.Structure):
@@ -70,7 +71,10 @@ def _load():
     lib.sacra_sommerfeld_rhs.argtypes = [vp, i32, vp, dp, dp, vp]
     lib.sacra_rk4_substep_bc.argtypes = [vp, i32, vp, vp, i32, dp, dp, dp, dp, vp]
     lib.sacra_rk4_step_bc.argtypes = [vp, i32, vp, vp, dp, dp, i64, vp]
-    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:16]:
+    lib.sacra_time_weights.argtypes = [i32, C.c_double, vp]
+    lib.sacra_lincomb.argtypes = [vp, i32, dp, dp, dp, vp, dp, vp]
+    lib.sacra_subcycle_step.argtypes = [vp, vp, vp, vp, vp, dp, dp, i32, dp, dp, i64, dp, i64, vp]
+    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:19]:
         getattr(lib, n).restype = C.c_int
     lib.sacra_strerror.argtypes = [C.c_int]
     lib.sacra_strerror.restype = C.c_char_p
@@ -246,3 +250,28 @@ def prolong_ghosts(parent, child, org, u_parent, u_child, stream=None):
     """6th-order Lagrange prolongation parent -> ghost cells of the child (sacra_prolong_ghosts)"""
     o = (C.c_int32 * 3)(*[int(v) for v in org]) if org is not None else None
     _check(lib.sacra_prolong_ghosts(_one(parent), _one(child), o, _ptr(u_parent), _ptr(u_child), _stream(stream)))
+
+
+def time_weights(nlevels, theta):
+    """weights of the parent time levels at theta (host function of the library)"""
+    w = (C.c_double * 3)()
+    _check(lib.sacra_time_weights(int(nlevels), float(theta), w))
+    return [w[0], w[1], w[2]]
+
+
+def lincomb(patch, levels, w, out, stream=None):
+    """out = (w0 u0 + w1 u1) [+ w2 u2] on every storage cell of one patch (sacra_lincomb)"""
+    n = len(levels)
+    u = list(levels) + [None] * (3 - n)
+    wv = (C.c_double * 3)(*([float(x) for x in w] + [0.0] * (3 - len(w))))
+    _check(lib.sacra_lincomb(_one(patch), n, _ptr(u[0]), _ptr(u[1]), _ptr(u[2]), wv, _ptr(out), _stream(stream)))
+
+
+def subcycle_step(parent, child, org, params, parent_bnd, u_parent, u_parent_prev, have_prev, u_child, work_parent,
+                  work_child, stream=None):
+    """one Berger-Oliger step of a parent / child pair (sacra_subcycle_step); work_parent: 5 parent states, work_child: 3"""
+    o = (C.c_int32 * 3)(*[int(v) for v in org]) if org is not None else None
+    pr = make_params(params) if params is not None else None
+    _check(lib.sacra_subcycle_step(_one(parent), _one(child), o, _ref(pr), make_boundaries([parent_bnd]), _ptr(u_parent),
+                                   _ptr(u_parent_prev), int(bool(have_prev)), _ptr(u_child), _ptr(work_parent),
+                                   int(u_parent.numel()), _ptr(work_child), int(u_child.numel()), _stream(stream)))

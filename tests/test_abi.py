@@ -169,3 +169,31 @@ def test_boundary_argument_checks():
     assert _code(sacra.rk4_substep_bc, ps, PRM, ok, 7, FAKE, FAKE, far, far + 8 * (total + 64)) == sacra.ERR_BADARG
     assert _code(sacra.rk4_step_bc, ps, PRM, ok, FAKE, FAKE + 64, total) == sacra.ERR_BADARG
     assert _code(sacra.rk4_step_bc, ps, PRM, None, FAKE, far, total) == sacra.ERR_NULL
+
+
+def test_subcycling_argument_checks():
+    pp, tp = wl.make_layout([(16, 16, 16)], [0.2], [0.05], [(0, 0, 0)])
+    pc, tc = wl.make_layout([(8, 8, 8)], [0.1], [0.025], [(0, 0, 0)])
+    slow, _ = wl.make_layout([(8, 8, 8)], [0.1], [0.05], [(0, 0, 0)])
+    assert sacra.time_weights(3, 0.5) == [-0.125, 0.75, 0.375]
+    assert sacra.time_weights(2, 0.25) == [0.75, 0.25, 0.0]
+    with pytest.raises(sacra.SacraError):
+        sacra.time_weights(4, 0.5)
+    step = 8 * (tp + 64)
+    bufs = [FAKE + k * 6 * step for k in range(5)]
+    bnd = ((0.0, 0.0, 0.0), [0] * 6)
+    class T:                                   # stand-in for a tensor: the binding only asks for numel() and the pointer
+        def __init__(self, ptr, n): self.ptr, self.n = ptr, n
+        def numel(self): return self.n
+    def call(parent, child, org, a, b, cc, d, e):
+        lib = sacra.lib
+        o = (C.c_int32 * 3)(*org)
+        return lib.sacra_subcycle_step(sacra.make_patches([parent]), sacra.make_patches([child]), o,
+                                       C.byref(sacra.make_params(PRM)), sacra.make_boundaries([bnd]), a, b, 0, cc, d, tp, e, tc, 0)
+    ok = (4, 4, 4)
+    assert call(pp[0], slow[0], ok, *bufs) == sacra.ERR_BADARG                 # the child's step is not dt / 2
+    assert call(pp[0], pc[0], (1, 4, 4), *bufs) == sacra.ERR_BADARG            # prolongation stencil leaves the parent
+    assert call(pp[0], pc[0], ok, bufs[0], bufs[0] + 64, *bufs[2:]) == sacra.ERR_BADARG   # overlapping buffers
+    assert call(pp[0], pc[0], ok, bufs[0], None, *bufs[2:]) == sacra.ERR_NULL
+    assert _code(sacra.lincomb, pp[0], [FAKE, FAKE + step], [0.5, 0.5], FAKE + 64) == sacra.ERR_BADARG
+    assert _code(sacra.lincomb, pp[0], [FAKE, None], [0.5, 0.5], FAKE + 2 * step) == sacra.ERR_NULL
