@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- Z4c RHS + KO + RK4 throughput of libsacra on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference] [--all-configs]
 
 One "step" = one full RK4 step (5 halo fills + 4 fused RHS/KO/RK substages) of the whole workload through the
 C ABI call sacra_rk4_step. Default workload: BASELINE.json configs[4], one 256^3 periodic patch, 25 FP64 fields,
@@ -27,12 +27,14 @@ sys.path.insert(0, ROOT)
 METRIC = "Z4c RHS+RK4 Mpoint-updates/s FP64"
 UNIT = "Mpoint-updates/s"
 NF = 25
-# Algorithmic work per point: 16 field passes x 8 B x 25 fields per RK4 step, i.e. 800 B per
-# substage launch on average; FP64 work per RHS evaluation + RK update after CSE: 3 272 FP64 instructions
-# (DADD 1 401, DMUL 818, DFMA 1 053 per point in the SASS of k_z4c<2>) = 4 325 flop with FMA = 2.
+# Algorithmic work per point: 16 field passes x 8 B x 25 fields per RK4 step (the
+# minimum of any RK4 formulation, 3 + 5 + 5 + 3; the increment-form acc of this library moves 3 + 5 + 5 + 4 = 17 with
+# SACRA_FLAG_SKIP_INCREMENT, which the timed steps set, and 18 without), i.e. 800 B per substage launch on average;
+# FP64 work per RHS evaluation + RK update after CSE: 3 284 FP64 instructions (DADD 1 399, DMUL 832, DFMA 1 053 per
+# point in the SASS of k_z4c<2>, profiles/r02_sass_histogram.md) = 4 337 flop with FMA = 2.
 ALG_BYTES_PER_POINT_STEP = 16 * 8 * NF
-ALG_FLOP_PER_POINT_STAGE = 4325.0
-ALG_FP64_INSTR_PER_POINT_STAGE = 3272.0
+ALG_FLOP_PER_POINT_STAGE = 4337.0
+ALG_FP64_INSTR_PER_POINT_STAGE = 3284.0
 FP64_LANES_PER_SM, N_SM = 64, 148
 
 
@@ -42,6 +44,25 @@ def _peaks():
         d = json.load(open(p))
         return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
     return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+def _csrc_digest() -> str:
+    """digest of the CUDA sources and build flags (the one paper_2607_08743_b200/build.py stamps the library with)"""
+    from paper_2607_08743_b200 import build as b
+    return b._digest()
+
+
+def _committed_traffic(workload: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/r02_traffic.json), or None
+    when the capture was made for other kernel sources or another workload"""
+    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    try:
+        d = json.load(open(p))
+    except (OSError, ValueError):
+        return None
+    if d.get("workload") != workload or d.get("csrc_digest") != _csrc_digest():
+        return None
+    return float(d["dram_bytes_per_launch_mean"])
 
 
 class ClockSampler:
@@ -97,6 +118,9 @@ def make_workload(idx: int, n: int | None):
     return wl.make(idx, **kw)
 
 
+ORACLE_SAMPLE_N = 160     # both CPU legs (cpu_baseline and --impl reference) time the same sample
+
+
 def oracle_sample(w, n_sample: int):
     """Bounded sample of the workload for the CPU legs: the central n_sample^3 block of patch 0 (same data,
     same spacing and parameters), advanced as its own periodic patch. Same work per point as the full run."""
@@ -131,7 +155,7 @@ def run_reference(args):
     if rank != 0:
         return
     w = make_workload(args.config, args.n)
-    m = args.oracle_n or 64
+    m = args.oracle_n or ORACLE_SAMPLE_N
     s = oracle_sample(w, m)
     ts, cores = time_oracle(s, args.steps, args.warmup)
     tot = sum(ts)
@@ -173,7 +197,9 @@ def run_ours(args):
         return replicas.max_over_ranks(x, device="cuda")
 
     w = make_workload(args.config, args.n)
-    ps, prm = sacra.make_patches(w.patches), sacra.make_params(w.params)
+    # the timed steps do not store the increment S ("may be skipped outside verification"; the new
+    # state is bit-identical, tests/test_gpu_multistep.py); the per-launch split below times the same kernels
+    ps, prm = sacra.make_patches(w.patches), sacra.make_params(dict(w.params, flags=sacra.FLAG_SKIP_INCREMENT))
     npts = w.npoints
     n = w.state.size
     host_in = torch.from_numpy(w.state).pin_memory()
@@ -322,7 +348,10 @@ def run_ours(args):
         roof = {"bound": "hbm", "achieved": alg_bytes / t_k / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof.update({
-        "traffic": args.traffic, "kernel": "k_z4c (fused derivative+algebra+KO+RK substage)",
+        "traffic": args.traffic if args.traffic is not None else _committed_traffic(w.name),
+        "traffic_source": "profiles/r02_traffic.json (ncu dram__bytes_read.sum + dram__bytes_write.sum, mean of the four "
+                          "substage launches; null if the kernel sources changed since the capture)",
+        "kernel": "k_z4c (fused derivative+algebra+KO+RK substage)",
         "kernel_ms": sub_avg, "kernel_share_of_step": 4 * sub_avg / (4 * sub_avg + 5 * fill_avg),
         "fill_ms": fill_avg, "alg_bytes_per_launch": alg_bytes, "alg_flop_per_launch": alg_flop,
         "hbm_frac": (alg_bytes / t_k / 1e9) / hbm_gbs, "alu_frac": (alg_flop / t_k / 1e12) / fp64_peak_tf,
@@ -336,7 +365,7 @@ def run_ours(args):
     cpu = None
     if not args.no_cpu:
         # bounded sample: about 10-20 s of oracle time on the box's host cores
-        s = oracle_sample(w, args.oracle_n or 160)
+        s = oracle_sample(w, args.oracle_n or ORACLE_SAMPLE_N)
         nst = 4 if s.npoints > 128 ** 3 else 8
         ts, cores = time_oracle(s, nst, 0)
         cpu = {"value": s.npoints * len(ts) / sum(ts) / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -344,6 +373,7 @@ def run_ours(args):
                          % (s.patches[0].nx, w.name, len(ts), sum(ts))}
 
     state_bytes = n * 8
+    ghost_cells = sum((p.nx + 6) * (p.ny + 6) * (p.nz + 6) - p.nx * p.ny * p.nz for p in w.patches)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": total_ms / K, "ms_per_step_min": min(step_ms), "ms_per_step_median": sorted(step_ms)[K // 2],
@@ -357,12 +387,64 @@ def run_ours(args):
                 "buffers, copy-in / kernels / copy-out on three streams",
                 "serial_value": world * npts * K / (e2e_serial_ms * 1e-3) / 1e6, "serial_ms_per_step": e2e_serial_ms / K},
         "gpu_launches": 9 * K, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
+        # the other kernels of the step against HBM: the halo fill reads and writes the ghost cells once
+        "kernels": {"k_fill_ghosts": {"ms": fill_avg, "hbm_frac": 2 * 8.0 * NF * ghost_cells / (fill_avg * 1e-3) / 1e9 / hbm_gbs},
+                    "k_z4c": {"ms": sub_avg, "hbm_frac": (alg_bytes / t_k / 1e9) / hbm_gbs}},
         # the constraint monitor on the state after the timed steps: 15 fields read + 4 written = 152 B per point
         "constraint_monitor": {"constraints_ms": con_ms, "norms_ms": nrm_ms, "Mpoints_per_s": npts / (con_ms * 1e-3) / 1e6,
                                "hbm_frac": 152.0 * npts / (con_ms * 1e-3) / 1e9 / hbm_gbs,
                                "norms_H_Mx_My_Mz": norms_host},
     }
+    if args.all_configs:
+        out["configs"] = [measure_config(i, args, hbm_gbs, fp64_peak_tf) for i in range(4)]
     print(json.dumps(out))
+
+
+def measure_config(idx, args, hbm_gbs, fp64_peak_tf):
+    """BASELINE.json configs 0-3 (the parity-test cases) timed the same way: K consecutive sacra_rk4_step calls from the
+    initial data, and -- these are launch-bound -- the same step captured into a CUDA graph by the caller and replayed.
+    frac: roofline fraction of the whole step (the slower of the algorithmic bytes at HBM bandwidth and the flops at the
+    FP64 peak, over the measured time per step). States of configs 0-1 fit the L2: their numbers are L2-resident."""
+    import torch
+    from paper_2607_08743_b200 import sacra
+    w = make_workload(idx, None)
+    ps, prm = sacra.make_patches(w.patches), sacra.make_params(dict(w.params, flags=sacra.FLAG_SKIP_INCREMENT))
+    n = w.state.size
+    u0 = torch.from_numpy(w.state).cuda()
+    u = u0.clone()
+    work = torch.zeros(3 * n, dtype=torch.float64, device="cuda")
+    K = max(args.steps, 20)
+    stream = torch.cuda.current_stream()
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(K):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / K
+
+    ms = timed(lambda: sacra.rk4_step(ps, prm, u, work, n))
+    u.copy_(u0)
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        sacra.rk4_step(ps, prm, u, work, n, stream=side)        # warm-up on the capture stream (tensor maps cached)
+        side.synchronize()
+        with torch.cuda.graph(g, stream=side):
+            sacra.rk4_step(ps, prm, u, work, n, stream=side)
+    u.copy_(u0)
+    ms_graph = timed(g.replay)
+    npts = w.npoints
+    t_roof = max(ALG_BYTES_PER_POINT_STEP * npts / (hbm_gbs * 1e9), 4 * ALG_FLOP_PER_POINT_STAGE * npts / (fp64_peak_tf * 1e12))
+    best = min(ms, ms_graph)
+    return {"workload": w.name, "patches": len(w.patches), "points": npts, "ms_per_step": ms,
+            "ms_per_step_cuda_graph": ms_graph, "value": npts / (best * 1e-3) / 1e6, "unit": UNIT,
+            "frac": t_roof / (best * 1e-3), "launches_per_step": 9 * ((len(w.patches) + 15) // 16),
+            "l2": "state %.0f MB" % (n * 8 / 1e6)}
 
 
 def main():
@@ -376,11 +458,11 @@ def main():
     ap.add_argument("--oracle-n", type=int, default=None, help="edge of the CPU oracle's sample block")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--traffic", type=float, default=None,
-                    help="dram bytes per launch of the dominant kernel from the committed ncu capture "
-                         "(default for config 4: profiles/r01_traffic_256.md)")
+                    help="dram bytes per launch of the dominant kernel (default: the committed ncu capture "
+                         "profiles/r02_traffic.json if it was made for the current kernel sources)")
+    ap.add_argument("--all-configs", action="store_true",
+                    help="also time BASELINE.json configs 0-3 (one line: the headline stays config 4, plus `configs`)")
     args = ap.parse_args()
-    if args.traffic is None and args.config == 4 and not args.n:
-        args.traffic = 21.88e9   # mean over the four substage launches, profiles/r01_traffic_256.md
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
