@@ -25,6 +25,7 @@ struct DevPatch {
   long long pitch, sz;     // doubles per x-row, doubles per z-plane
   long long fstride, offset;
   double dx, dt;
+  GridCoef gc;             // 1/(12 h) ... of the derivative stage (launch_z4c fills in the KO factor)
   unsigned shell;          // bit 2a + side: that face is a Sommerfeld face (its 3 outermost layers are the boundary shell)
 };
 struct PatchBatch {
@@ -364,8 +365,8 @@ __global__ void __launch_bounds__(Tile::NTH, 1) k_z4c(const __grid_constant__ Pa
       const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
       Emitter<(EPI < 0 ? 0 : EPI), Src> emit{src, rhs, rk.u_out, rk.acc, p.offset + c, p.fstride, p.dt, active};
       src.begin_tile();
-      if constexpr (EPI < 0) constraints_point(src, p.dx, emit);
-      else z4c_point(src, P, p.dx, emit);
+      if constexpr (EPI < 0) constraints_point(src, p.gc, emit);
+      else z4c_point(src, P, p.gc, emit);
       if (!src.has_next) break;
       t = tn;
       id = desc[(iter + 1) & 1u];   // written by the producer at the top of this tile
@@ -583,6 +584,7 @@ static DevPatch to_dev(const sacra_patch_t& a) {
   d.pitch = a.pitch_x; d.sz = a.pitch_x * (long long)(a.ny + 2 * NG);
   d.fstride = a.field_stride; d.offset = a.patch_offset; d.dx = a.dx; d.dt = a.dt;
   d.shell = 0;
+  d.gc = grid_coef(a.dx, 0.0);
   return d;
 }
 
@@ -776,6 +778,7 @@ static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* 
     for (int q = 0; q < B.np; ++q) {
       const sacra_patch_t& a = p[q0 + q];
       B.p[q] = to_dev(a);
+      B.p[q].gc = grid_coef(a.dx, prm->ko_sigma);
       if (bnd) B.p[q].shell = shell_bits(bnd[q0 + q]);
       B.first_block[q] = nb;
       nb += ((a.nx + Tile::TX - 1) / Tile::TX) * ((a.ny + Tile::TY - 1) / Tile::TY) * ((a.nz + Tile::TZ - 1) / Tile::TZ);

@@ -19,12 +19,12 @@
 namespace sacra {
 
 template <class Src, class Emit>
-__device__ __forceinline__ void constraints_point(const Src& src, double h, Emit& emit) {
+__device__ __forceinline__ void constraints_point(const Src& src, const GridCoef& gc, Emit& emit) {
   Stencil S;
   PointCoef pc;
   {
     const double zero[3] = {0.0, 0.0, 0.0};
-    make_coef(h, 0.0, zero, pc);
+    make_coef(gc, zero, pc);
   }
   // ---- centre values first (Tensor Memory strip): metric, its inverse, K, B_ij = At_ij + gt_ij K / 3 ----------------
   double g[6], gi[6], A[6], Kh, Th;

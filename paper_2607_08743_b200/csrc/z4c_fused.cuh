@@ -54,7 +54,7 @@ __device__ __forceinline__ double tr_fma(const double (&a)[6], const double (&b)
 }
 
 template <class Src, class Emit>
-__device__ __forceinline__ void z4c_point(const Src& src, const Params& P, double h, Emit& emit) {
+__device__ __forceinline__ void z4c_point(const Src& src, const Params& P, const GridCoef& gc, Emit& emit) {
   using namespace tmem;
   const double half = 0.5, third = 1.0 / 3.0, two3 = 2.0 / 3.0;
   Stencil S;
@@ -73,7 +73,7 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, doubl
     Kh = p8.get(3);
     Bc[0] = p12.get(0); Bc[1] = p12.get(1); Bc[2] = p12.get(2);
     Th = p12.get(3);
-    make_coef(h, P.ko_sigma, beta, pc);
+    make_coef(gc, beta, pc);
   }
   {
     const double gxx = g[0], gxy = g[1], gxz = g[2], gyy = g[3], gyz = g[4], gzz = g[5];

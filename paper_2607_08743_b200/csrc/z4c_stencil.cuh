@@ -34,16 +34,29 @@ struct PointCoef {      // per-thread constants of the derivative stage
   double bs[3];         // |beta^a| / (24 h)  weight of its symmetric part
 };
 
-__device__ __forceinline__ void make_coef(double h, double sigma, const double (&beta)[3], PointCoef& c) {
-  c.inv12h = 1.0 / (12.0 * h);
-  c.inv12h2 = 1.0 / ((12.0 * h) * h);
-  c.inv144h2 = 1.0 / ((144.0 * h) * h);
-  c.kofac = sigma / (64.0 * h);
-  const double inv24h = 1.0 / (24.0 * h);
+// per-patch constants of the derivative stage, computed once on the host (IEEE double, the same expressions the
+// oracle evaluates: identical bits) instead of five divisions per thread and tile
+struct GridCoef {
+  double inv12h, inv12h2, inv144h2, inv24h, kofac;
+};
+__host__ __device__ __forceinline__ GridCoef grid_coef(double h, double sigma) {
+  GridCoef g;
+  g.inv12h = 1.0 / (12.0 * h);
+  g.inv12h2 = 1.0 / ((12.0 * h) * h);
+  g.inv144h2 = 1.0 / ((144.0 * h) * h);
+  g.inv24h = 1.0 / (24.0 * h);
+  g.kofac = sigma / (64.0 * h);
+  return g;
+}
+__device__ __forceinline__ void make_coef(const GridCoef& g, const double (&beta)[3], PointCoef& c) {
+  c.inv12h = g.inv12h;
+  c.inv12h2 = g.inv12h2;
+  c.inv144h2 = g.inv144h2;
+  c.kofac = g.kofac;
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
-    c.ba[a] = beta[a] * inv24h;
-    c.bs[a] = fabs(beta[a]) * inv24h;
+    c.ba[a] = beta[a] * g.inv24h;
+    c.bs[a] = fabs(beta[a]) * g.inv24h;
   }
 }
 
