@@ -223,6 +223,20 @@ int sacra_subcycle_step(const sacra_patch_t* parent, const sacra_patch_t* child,
                         double* u_parent_prev, int have_prev, double* u_child, double* work_parent,
                         int64_t parent_doubles, double* work_child, int64_t child_doubles, void* cuda_stream);
 
+/* Halo exchange between the patches of a block decomposition over several GPUs (the
+ * 3 ghost layers of every field at every face are packed into a buffer and exchanged with the neighbouring rank before
+ * each RK substage). ONE patch per call. axis 0, 1, 2 = x, y, z; side 0 = low face, 1 = high face.
+ *   sacra_face_doubles   doubles in a face buffer of the axis: 25 fields x 3 layers x the whole STORAGE extent of the two
+ *                        other axes (their ghost cells travel too: exchanging x, then y, then z fills edges and corners).
+ *   sacra_pack_face      buf <- the 3 outermost ACTIVE layers at the face, layout [field][layer][slower][faster] (layer
+ *                        and the two other axes in increasing storage index).
+ *   sacra_unpack_face    the 3 GHOST layers behind the face <- buf (same layout). The buffer a rank packs at its high
+ *                        face is what its high neighbour unpacks at its low face, and vice versa.
+ * The transfer itself is the caller's (paper_2607_08743_b200/halo.py: torch.distributed point-to-point over NCCL). */
+int64_t sacra_face_doubles(const sacra_patch_t* p, int axis);
+int sacra_pack_face(const sacra_patch_t* p, const double* u, int axis, int side, double* buf, void* cuda_stream);
+int sacra_unpack_face(const sacra_patch_t* p, double* u, int axis, int side, const double* buf, void* cuda_stream);
+
 /* Static description of a status code (never NULL). */
 const char* sacra_strerror(int code);
 

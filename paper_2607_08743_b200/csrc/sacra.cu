@@ -521,6 +521,28 @@ __global__ void __launch_bounds__(128) k_prolong_ghosts(const __grid_constant__ 
   u_child[pc.offset + (long long)blockIdx.y * pc.fstride + (long long)Kk * pc.sz + (long long)J * pc.pitch + I] = az;
 }
 
+// Halo exchange between the patches of a block decomposition ("pack, then non-blocking
+// GPU-aware exchange"): the NG outermost ACTIVE layers at a face go into a contiguous buffer [field][layer][row][col]
+// (the two other axes over their whole STORAGE extent, so that exchanging x, then y, then z also fills edges and
+// corners), and a received buffer goes into the NG GHOST layers of a face. PACK: true = pack, false = unpack.
+template <bool PACK>
+__global__ void __launch_bounds__(256) k_face(const __grid_constant__ DevPatch p, int axis, int side,
+                                              double* __restrict__ u, double* __restrict__ buf) {
+  const int s[3] = {p.nx + 2 * NG, p.ny + 2 * NG, p.nz + 2 * NG}, n[3] = {p.nx, p.ny, p.nz};
+  const int a1 = axis == 0 ? 1 : 0, a2 = axis == 2 ? 1 : 2;       // the other two axes, the faster one first
+  const long long st[3] = {1, p.pitch, p.sz};
+  const int f = blockIdx.y, l = blockIdx.x;                          // field, layer
+  // storage index of the layer: active layers [NG, 2NG) / [n, n + NG) when packing, ghost layers when unpacking
+  const int L = PACK ? (side == 0 ? NG + l : n[axis] + l) : (side == 0 ? l : n[axis] + NG + l);
+  double* base = u + p.offset + (long long)f * p.fstride + (long long)L * st[axis];
+  double* b = buf + ((long long)f * NG + l) * s[a1] * s[a2];
+  for (int q = threadIdx.x + blockDim.x * blockIdx.z; q < s[a1] * s[a2]; q += blockDim.x * gridDim.z) {
+    const long long c = (long long)(q % s[a1]) * st[a1] + (long long)(q / s[a1]) * st[a2];
+    if (PACK) b[q] = base[c];
+    else base[c] = b[q];
+  }
+}
+
 // linear combination of up to three states on every storage cell of a patch (time interpolation of the parent levels,
 // SURVEY 8(f) f-3): out = (w0 u0 + w1 u1) [+ w2 u2], one rounding per operation like the oracle's
 struct LinComb {
@@ -1041,6 +1063,33 @@ int sacra_prolong_ghosts(const sacra_patch_t* parent, const sacra_patch_t* child
   const int n = 2 * NG * (sx * sy + sx * child->nz + child->ny * child->nz);   // cells of the ghost shell
   k_prolong_ghosts<<<dim3((n + 127) / 128, NF), 128, 0, static_cast<cudaStream_t>(cuda_stream)>>>(L, u_parent, u_child);
   return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
+}
+
+int64_t sacra_face_doubles(const sacra_patch_t* p, int axis) {
+  if (!p || axis < 0 || axis > 2) return 0;
+  const int64_t s[3] = {p->nx + 2 * SACRA_NG, p->ny + 2 * SACRA_NG, p->nz + 2 * SACRA_NG};
+  return (int64_t)SACRA_NF * SACRA_NG * (s[0] * s[1] * s[2] / s[axis]);
+}
+
+static int face_call(bool pack, const sacra_patch_t* p, double* u, int axis, int side, double* buf, void* cuda_stream) {
+  if (!p || !u || !buf) return SACRA_ERR_NULL;
+  if (int e = check_patches(p, 1)) return e;
+  if (axis < 0 || axis > 2 || side < 0 || side > 1) return SACRA_ERR_BADARG;
+  if (!aligned16(u) || !aligned16(buf)) return SACRA_ERR_ALIGN;
+  if (overlap(u, state_extent(p, 1), buf, sacra_face_doubles(p, axis))) return SACRA_ERR_BADARG;
+  const long long plane = sacra_face_doubles(p, axis) / (SACRA_NF * SACRA_NG);
+  const int split = plane / 16384 < 1 ? 1 : (plane / 16384 > 8 ? 8 : (int)(plane / 16384));
+  const dim3 grid(NG, NF, split);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (pack) k_face<true><<<grid, 256, 0, st>>>(to_dev(*p), axis, side, u, buf);
+  else k_face<false><<<grid, 256, 0, st>>>(to_dev(*p), axis, side, u, buf);
+  return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
+}
+int sacra_pack_face(const sacra_patch_t* p, const double* u, int axis, int side, double* buf, void* cuda_stream) {
+  return face_call(true, p, const_cast<double*>(u), axis, side, buf, cuda_stream);
+}
+int sacra_unpack_face(const sacra_patch_t* p, double* u, int axis, int side, const double* buf, void* cuda_stream) {
+  return face_call(false, p, u, axis, side, const_cast<double*>(buf), cuda_stream);
 }
 
 int sacra_time_weights(int nlevels, double theta, double* w) {

@@ -23,7 +23,8 @@ EXPORTS = ("sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4
            "sacra_constraints", "sacra_constraint_norms", "sacra_constraint_scratch_doubles",
            "sacra_fill_ghosts_bc", "sacra_restrict", "sacra_prolong_ghosts",
            "sacra_fill_ghosts_faces", "sacra_sommerfeld_rhs", "sacra_rk4_substep_bc", "sacra_rk4_step_bc",
-           "sacra_time_weights", "sacra_lincomb", "sacra_subcycle_step")
+           "sacra_time_weights", "sacra_lincomb", "sacra_subcycle_step",
+           "sacra_face_doubles", "sacra_pack_face", "sacra_unpack_face")
 
 
 class SacraPatch(C.Structure):
@@ -74,7 +75,11 @@ def _load():
     lib.sacra_time_weights.argtypes = [i32, C.c_double, vp]
     lib.sacra_lincomb.argtypes = [vp, i32, dp, dp, dp, vp, dp, vp]
     lib.sacra_subcycle_step.argtypes = [vp, vp, vp, vp, vp, dp, dp, i32, dp, dp, i64, dp, i64, vp]
-    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:19]:
+    lib.sacra_face_doubles.argtypes = [vp, i32]
+    lib.sacra_face_doubles.restype = C.c_int64
+    lib.sacra_pack_face.argtypes = [vp, dp, i32, i32, dp, vp]
+    lib.sacra_unpack_face.argtypes = [vp, dp, i32, i32, dp, vp]
+    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:19] + EXPORTS[20:22]:
         getattr(lib, n).restype = C.c_int
     lib.sacra_strerror.argtypes = [C.c_int]
     lib.sacra_strerror.restype = C.c_char_p
@@ -275,3 +280,17 @@ def subcycle_step(parent, child, org, params, parent_bnd, u_parent, u_parent_pre
     _check(lib.sacra_subcycle_step(_one(parent), _one(child), o, _ref(pr), make_boundaries([parent_bnd]), _ptr(u_parent),
                                    _ptr(u_parent_prev), int(bool(have_prev)), _ptr(u_child), _ptr(work_parent),
                                    int(u_parent.numel()), _ptr(work_child), int(u_child.numel()), _stream(stream)))
+
+
+def face_doubles(patch, axis) -> int:
+    return int(lib.sacra_face_doubles(_one(patch), int(axis)))
+
+
+def pack_face(patch, u, axis, side, buf, stream=None):
+    """buf <- the 3 outermost active layers at a face (sacra_pack_face)"""
+    _check(lib.sacra_pack_face(_one(patch), _ptr(u), int(axis), int(side), _ptr(buf), _stream(stream)))
+
+
+def unpack_face(patch, u, axis, side, buf, stream=None):
+    """the 3 ghost layers behind a face <- buf (sacra_unpack_face)"""
+    _check(lib.sacra_unpack_face(_one(patch), _ptr(u), int(axis), int(side), _ptr(buf), _stream(stream)))

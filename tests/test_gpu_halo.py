@@ -1,0 +1,58 @@
+"""-m gpu: the pack / unpack kernels of the halo exchange against the buffer layout sacra.h states, and
+the single-rank exchange (every axis its own neighbour) against sacra_fill_ghosts, bit for bit; one distributed RK4
+step on a 1 x 1 x 1 topology equals sacra_rk4_step bitwise."""
+import numpy as np
+import pytest
+import torch
+
+from gpu_util import dev, host
+from helpers import NF, NG
+from paper_2607_08743_b200 import halo, sacra
+from paper_2607_08743_b200 import workloads as wl
+from test_halo_gloo import NumpyOps
+
+pytestmark = pytest.mark.gpu
+
+
+def _w(dims=(11, 8, 9), seed=2):
+    ps, total = wl.make_layout([dims], [0.1], [0.02], [(0, 0, 0)])
+    return wl.Workload("h", ps, dict(wl.DEFAULT_PARAMS), np.random.default_rng(seed).normal(size=total))
+
+
+def test_pack_and_unpack_follow_the_stated_layout():
+    w = _w()
+    p = w.patches[0]
+    ref_ops = NumpyOps(w)
+    u = dev(w.state)
+    for axis in range(3):
+        assert sacra.face_doubles(p, axis) == ref_ops.new_buffer(p, axis, None).numel()
+        for side in (0, 1):
+            buf = torch.zeros(sacra.face_doubles(p, axis), dtype=torch.float64, device="cuda")
+            sacra.pack_face(p, u, axis, side, buf)
+            ref = ref_ops.new_buffer(p, axis, None)
+            ref_ops.pack(p, torch.from_numpy(w.state), axis, side, ref)
+            assert np.array_equal(host(buf), ref.numpy()), (axis, side)
+            tgt, tgt_ref = dev(w.state), torch.from_numpy(w.state.copy())
+            sacra.unpack_face(p, tgt, axis, side, buf)
+            ref_ops.unpack(p, tgt_ref, axis, side, ref)
+            assert np.array_equal(host(tgt), tgt_ref.numpy()), (axis, side)
+
+
+def test_single_rank_exchange_equals_periodic_fill_and_step():
+    w = _w((13, 9, 10), seed=3)
+    for f in range(NF):
+        a = w.active_view(w.state, 0, f)
+        a *= 0.01
+        if f in (wl.F_W, wl.F_G, wl.F_G + 3, wl.F_G + 5, wl.F_ALP):
+            a += 1.0
+    p = w.patches[0]
+    topo = halo.CartTopology((1, 1, 1))
+    u, v = dev(w.state), dev(w.state)
+    assert halo.exchange_halos(p, u, topo, 0) == 0
+    sacra.fill_ghosts([p], v)
+    assert np.array_equal(host(u), host(v))
+    n = u.numel()
+    wu, wv = torch.zeros(3 * n, dtype=torch.float64, device="cuda"), torch.zeros(3 * n, dtype=torch.float64, device="cuda")
+    halo.rk4_step_distributed(p, w.params, u, wu, topo, 0)
+    sacra.rk4_step([p], w.params, v, wv)
+    assert np.array_equal(host(u), host(v)) and np.array_equal(host(wu[2 * n:]), host(wv[2 * n:]))
