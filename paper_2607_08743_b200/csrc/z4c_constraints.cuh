@@ -55,22 +55,23 @@ __device__ __forceinline__ void constraints_point(const Src& src, const GridCoef
   for (int n = 0; n < 6; ++n) B[n] = A[n] + g[n] * K / 3.0;
 
   // ---- derivatives, field by field; second derivatives of gt_ij and the gradient of B_ij are folded at once -------
-  double dW[3], ddW[6];
+  // the derivatives that are only needed at the very end (d_k W, d_i d_j W, d_k gt_ij) wait in the Tensor Memory
+  // strip (slots of z4c_tile.cuh: PK_DB 12 doubles, PK_DG 6 groups of 4), not in registers
+  using namespace tmem;
   field_derivs<true, true, false>(src.template field<F_W>(), pc, S);
   const double W = S.u0;
-#pragma unroll
-  for (int k = 0; k < 3; ++k) dW[k] = S.d1[k];
-#pragma unroll
-  for (int n = 0; n < 6; ++n) ddW[n] = S.d2[n];
+  st4(src.strip(PK_DB), S.d1[0], S.d1[1], S.d1[2], S.d2[0]);
+  st4(src.strip(PK_DB + 4), S.d2[1], S.d2[2], S.d2[3], S.d2[4]);
+  st1(src.strip(PK_DB + 8), S.d2[5]);
 
   // second-derivative part of the Ricci scalar of gt:  gt^ij gt^kl ( d_k d_i gt_lj - d_k d_l gt_ij ); the field
   // gt_ab contributes  m_ab [ (gt^.a)^T D2 (gt^.b) - gt^ab tr(gt^-1 D2) ],  m_ab = 1 (a = b) or 2
-  double dg[3][6], R2 = 0.0;
+  double R2 = 0.0;
 #define GT_FIELD(A, Bx)                                                                             \
   {                                                                                                 \
     constexpr int N = sym(A, Bx);                                                                   \
     field_derivs<true, true, false>(src.template field<F_G + N>(), pc, S);                          \
-    _Pragma("unroll") for (int k = 0; k < 3; ++k) dg[k][N] = S.d1[k];                               \
+    st4(src.strip(PK_DG + 4 * N), S.d1[0], S.d1[1], S.d1[2], 0.0);                                  \
     double q = 0.0, tr = 0.0;                                                                       \
     _Pragma("unroll") for (int i = 0; i < 3; ++i)                                                   \
       _Pragma("unroll") for (int k = 0; k < 3; ++k) {                                               \
@@ -82,6 +83,7 @@ __device__ __forceinline__ void constraints_point(const Src& src, const GridCoef
   GT_FIELD(0, 0) GT_FIELD(0, 1) GT_FIELD(0, 2) GT_FIELD(1, 1) GT_FIELD(1, 2) GT_FIELD(2, 2)
 #undef GT_FIELD
 
+  wait_st();            // the parked derivatives are read back from here on
   double dK[3];
   field_derivs<true, false, false>(src.template field<F_KH>(), pc, S);
 #pragma unroll
@@ -96,9 +98,12 @@ __device__ __forceinline__ void constraints_point(const Src& src, const GridCoef
 #define AT_FIELD(A, Bx)                                                                             \
   {                                                                                                 \
     constexpr int N = sym(A, Bx);                                                                   \
+    Pack4 dgn;                                                                                      \
+    ld4(src.strip(PK_DG + 4 * N), dgn);                                                             \
     field_derivs<true, false, false>(src.template field<F_A + N>(), pc, S);                         \
+    wait_ld(dgn);                                                                                   \
     double dBn[3];                                                                                  \
-    _Pragma("unroll") for (int k = 0; k < 3; ++k) dBn[k] = S.d1[k] + (dg[k][N] * K + g[N] * dK[k]) / 3.0; \
+    _Pragma("unroll") for (int k = 0; k < 3; ++k) dBn[k] = S.d1[k] + (dgn.get(k) * K + g[N] * dK[k]) / 3.0; \
     const double va = (gi[sym(0, A)] * dBn[0] + gi[sym(1, A)] * dBn[1]) + gi[sym(2, A)] * dBn[2];   \
     const double vb = (gi[sym(0, Bx)] * dBn[0] + gi[sym(1, Bx)] * dBn[1]) + gi[sym(2, Bx)] * dBn[2]; \
     _Pragma("unroll") for (int i = 0; i < 3; ++i)                                                   \
@@ -107,6 +112,22 @@ __device__ __forceinline__ void constraints_point(const Src& src, const GridCoef
   AT_FIELD(0, 0) AT_FIELD(0, 1) AT_FIELD(0, 2) AT_FIELD(1, 1) AT_FIELD(1, 2) AT_FIELD(2, 2)
 #undef AT_FIELD
 
+  // ---- the parked derivatives come back ----------------------------------------------------------------------------
+  double dg[3][6], dW[3], ddW[6];
+  {
+    Pack4 q[6], w0, w4;
+    Pack1 w8;
+#pragma unroll
+    for (int n = 0; n < 6; ++n) ld4(src.strip(PK_DG + 4 * n), q[n]);
+    ld4(src.strip(PK_DB), w0); ld4(src.strip(PK_DB + 4), w4); ld1(src.strip(PK_DB + 8), w8);
+    wait_ld(q[0], q[1], q[2], q[3], q[4], q[5], w0, w4, w8);
+#pragma unroll
+    for (int n = 0; n < 6; ++n)
+#pragma unroll
+      for (int k = 0; k < 3; ++k) dg[k][n] = q[n].get(k);
+    dW[0] = w0.get(0); dW[1] = w0.get(1); dW[2] = w0.get(2);
+    ddW[0] = w0.get(3); ddW[1] = w4.get(0); ddW[2] = w4.get(1); ddW[3] = w4.get(2); ddW[4] = w4.get(3); ddW[5] = w8.get(0);
+  }
   // ---- gradient of the inverse conformal metric -----------------------------------------------------------------
   double dgi[3][6];                   // d_l gt^ij = - gt^ia gt^jb d_l gt_ab
 #pragma unroll
