@@ -128,21 +128,22 @@ __device__ __forceinline__ void constraints_point(const Src& src, const GridCoef
     dW[0] = w0.get(0); dW[1] = w0.get(1); dW[2] = w0.get(2);
     ddW[0] = w0.get(3); ddW[1] = w4.get(0); ddW[2] = w4.get(1); ddW[3] = w4.get(2); ddW[4] = w4.get(3); ddW[5] = w8.get(0);
   }
-  // ---- gradient of the inverse conformal metric -----------------------------------------------------------------
-  double dgi[3][6];                   // d_l gt^ij = - gt^ia gt^jb d_l gt_ab
+  // ---- gradient of the inverse conformal metric: d_l gt^ij = -(gt^-1 d_l gt gt^-1)^ij, two 3 x 3 products per l -------
+  double dgi[3][6];
 #pragma unroll
-  for (int l = 0; l < 3; ++l)
+  for (int l = 0; l < 3; ++l) {
+    double t[3][3];                   // t[i][b] = gt^ia d_l gt_ab
 #pragma unroll
     for (int i = 0; i < 3; ++i)
 #pragma unroll
-      for (int j = i; j < 3; ++j) {
-        double s = 0.0;
+      for (int bb = 0; bb < 3; ++bb)
+        t[i][bb] = fma(gi[sym(i, 2)], dg[l][sym(2, bb)], fma(gi[sym(i, 1)], dg[l][sym(1, bb)], gi[sym(i, 0)] * dg[l][sym(0, bb)]));
 #pragma unroll
-        for (int a = 0; a < 3; ++a)
+    for (int i = 0; i < 3; ++i)
 #pragma unroll
-          for (int b = 0; b < 3; ++b) s += gi[sym(i, a)] * gi[sym(j, b)] * dg[l][sym(a, b)];
-        dgi[l][sym(i, j)] = -s;
-      }
+      for (int j = i; j < 3; ++j)
+        dgi[l][sym(i, j)] = -fma(t[i][2], gi[sym(2, j)], fma(t[i][1], gi[sym(1, j)], t[i][0] * gi[sym(0, j)]));
+  }
   // ---- Christoffel symbols of gt: Gl[c][ij] first kind, Gu[k][ij] second kind -----------------------------------
   double Gl[3][6], Gu[3][6];
 #pragma unroll
@@ -157,22 +158,39 @@ __device__ __forceinline__ void constraints_point(const Src& src, const GridCoef
     for (int n = 0; n < 6; ++n) Gu[k][n] = (gi[sym(k, 0)] * Gl[0][n] + gi[sym(k, 1)] * Gl[1][n]) + gi[sym(k, 2)] * Gl[2][n];
 
   // ---- Ricci scalar of gt: the folded second-derivative part + the first-derivative terms of
-  //      gt^ij ( d_k Gt^k_ij - d_j Gt^k_ik + Gt^k_kl Gt^l_ij - Gt^k_jl Gt^l_ik ) ---------------------------------------
+  //      gt^ij ( d_k Gt^k_ij - d_j Gt^k_ik + Gt^k_kl Gt^l_ij - Gt^k_jl Gt^l_ik ),  d gt^kl Gt_l,ij standing for the
+  //      part of d Gt^k_ij without second derivatives. Contracted intermediates instead of the four-fold loop:
+  //        a_l = d_k gt^kl,  c_l = Gt^k_kl                     ->  sum_l (a_l + ...) of  gt^ij Gt_l,ij  and  gt^ij Gt^l_ij
+  //        P[i][k][l] = gt^ij d_j gt^kl,  H[i][k][l] = gt^ij Gt^k_jl   ->  - P[i][k][l] Gt_l,ik  -  H[i][k][l] Gt^l_ik
   double Rt = R2;
+  {
+    double trl[3], tru[3];            // gt^ij Gt_l,ij ,  gt^ij Gt^l_ij
 #pragma unroll
-  for (int i = 0; i < 3; ++i)
+    for (int l = 0; l < 3; ++l) {
+      double d = fma(gi[5], Gl[l][5], fma(gi[3], Gl[l][3], gi[0] * Gl[l][0]));
+      double o = fma(gi[4], Gl[l][4], fma(gi[2], Gl[l][2], gi[1] * Gl[l][1]));
+      trl[l] = fma(2.0, o, d);
+      d = fma(gi[5], Gu[l][5], fma(gi[3], Gu[l][3], gi[0] * Gu[l][0]));
+      o = fma(gi[4], Gu[l][4], fma(gi[2], Gu[l][2], gi[1] * Gu[l][1]));
+      tru[l] = fma(2.0, o, d);
+    }
 #pragma unroll
-    for (int j = 0; j < 3; ++j) {
-      double r = 0.0;
+    for (int l = 0; l < 3; ++l) {
+      const double al = (dgi[0][sym(0, l)] + dgi[1][sym(1, l)]) + dgi[2][sym(2, l)];
+      const double cl = (Gu[0][sym(0, l)] + Gu[1][sym(1, l)]) + Gu[2][sym(2, l)];
+      Rt = fma(al, trl[l], fma(cl, tru[l], Rt));
+    }
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
 #pragma unroll
       for (int k = 0; k < 3; ++k)
 #pragma unroll
         for (int l = 0; l < 3; ++l) {
-          r += dgi[k][sym(k, l)] * Gl[l][sym(i, j)] - dgi[j][sym(k, l)] * Gl[l][sym(i, k)];
-          r += Gu[k][sym(k, l)] * Gu[l][sym(i, j)] - Gu[k][sym(j, l)] * Gu[l][sym(i, k)];
+          const double Pikl = fma(gi[sym(i, 2)], dgi[2][sym(k, l)], fma(gi[sym(i, 1)], dgi[1][sym(k, l)], gi[sym(i, 0)] * dgi[0][sym(k, l)]));
+          const double Hikl = fma(gi[sym(i, 2)], Gu[k][sym(2, l)], fma(gi[sym(i, 1)], Gu[k][sym(1, l)], gi[sym(i, 0)] * Gu[k][sym(0, l)]));
+          Rt = fma(-Pikl, Gl[l][sym(i, k)], fma(-Hikl, Gu[l][sym(i, k)], Rt));
         }
-      Rt += gi[sym(i, j)] * r;
-    }
+  }
   // ---- conformal factor: R = W^2 Rt + 4 W Dt^2 W - 6 |Dt W|^2 -----------------------------------------------------
   double lapW = 0.0, dWdW = 0.0;
 #pragma unroll
@@ -204,23 +222,32 @@ __device__ __forceinline__ void constraints_point(const Src& src, const GridCoef
   for (int j = 0; j < 3; ++j) w[j] = dW[j] / W;
 #pragma unroll
   for (int c = 0; c < 3; ++c) wu[c] = (gi[sym(c, 0)] * w[0] + gi[sym(c, 1)] * w[1]) + gi[sym(c, 2)] * w[2];
+  // full connection Gamma^c_ja = Gt^c_ja + C^c_ja ,  C^c_ja = -( delta^c_j w_a + delta^c_a w_j - gt_ja w^c ), formed once;
+  // cov_jab = -2 w_j B_ab - Gamma^c_ja B_cb - Gamma^c_jb B_ac (the gradient d_j B_ab is already in M);
+  // M^i += gt^ia ( gt^jb cov_jab ): contracted over (j, b) first
+  double Gf[3][6];
 #pragma unroll
-  for (int j = 0; j < 3; ++j)
+  for (int c = 0; c < 3; ++c)
 #pragma unroll
-    for (int a = 0; a < 3; ++a)
+    for (int j = 0; j < 3; ++j)
+#pragma unroll
+      for (int a = j; a < 3; ++a)
+        Gf[c][sym(j, a)] = Gu[c][sym(j, a)] - ((((c == j) ? w[a] : 0.0) + ((c == a) ? w[j] : 0.0)) - g[sym(j, a)] * wu[c]);
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    double va = 0.0;                  // gt^jb cov_jab
+#pragma unroll
+    for (int j = 0; j < 3; ++j)
 #pragma unroll
       for (int b = 0; b < 3; ++b) {
-        double cov = -2.0 * w[j] * B[sym(a, b)];   // the gradient d_j B_ab is already in M
+        double cov = -2.0 * w[j] * B[sym(a, b)];
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          // Gamma^c_ja = Gt^c_ja + C^c_ja ,  C^c_ja = -( delta^c_j w_a + delta^c_a w_j - gt_ja w^c )
-          const double Cja = -(((c == j) ? w[a] : 0.0) + ((c == a) ? w[j] : 0.0) - g[sym(j, a)] * wu[c]);
-          const double Cjb = -(((c == j) ? w[b] : 0.0) + ((c == b) ? w[j] : 0.0) - g[sym(j, b)] * wu[c]);
-          cov -= (Gu[c][sym(j, a)] + Cja) * B[sym(c, b)] + (Gu[c][sym(j, b)] + Cjb) * B[sym(a, c)];
-        }
-#pragma unroll
-        for (int i = 0; i < 3; ++i) M[i] += gi[sym(i, a)] * gi[sym(j, b)] * cov;
+        for (int c = 0; c < 3; ++c) cov = fma(-Gf[c][sym(j, a)], B[sym(c, b)], fma(-Gf[c][sym(j, b)], B[sym(a, c)], cov));
+        va = fma(gi[sym(j, b)], cov, va);
       }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) M[i] = fma(gi[sym(i, a)], va, M[i]);
+  }
 #pragma unroll
   for (int i = 0; i < 3; ++i) M[i] -= (gi[sym(i, 0)] * dK[0] + gi[sym(i, 1)] * dK[1]) + gi[sym(i, 2)] * dK[2];
   emit.template put<1>(W * W * M[0], 0.0);
