@@ -22,9 +22,11 @@
 //   -fno-fast-math, -ffp-contract=off
 // Readings of silent / garbled points are listed in DESIGN.md ("Readings").
 //
-// PARITY UNPINNED: (C) whether Eq. 6's source is K-hat or
-// K-hat+2*Theta (switch lapse_uses_khat); the kappa1/kappa2 coefficient
-// placement beyond the uniform-Theta decay-rate check.
+// PARITY UNPINNED with respect to the paper: (C) whether
+// Eq. 6's source is K-hat or K-hat+2*Theta (switch lapse_uses_khat); the placement
+// of the kappa1/kappa2 coefficients. Both are pinned against SURVEY.md 8(c)'s
+// linear-response table (tests/test_oracle_linear_response.py), and the Theta
+// coefficient against the constraint monitor; the paper itself prints neither.
 //
 // Everything is templated on the scalar type so that the same source builds
 // as double (the oracle) and as __float128 (round-off referee).

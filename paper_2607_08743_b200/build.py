@@ -3,8 +3,8 @@
     python -m paper_2607_08743_b200.build [--force] [--verbose]   ->  paper_2607_08743_b200/libsacra.so
 
 nvcc cross-compiles without a GPU. -lineinfo keeps the ncu source page usable. No --use_fast_math
-(-fno-fast-math on every platform); FMA contraction is controlled per expression in the
-sources (stencils use __dadd_rn/__dmul_rn and are never contracted).
+(-fno-fast-math on every platform) and -fmad=false: an FMA appears only where the
+sources write fma() explicitly (csrc/z4c_stencil.cuh, z4c_fused.cuh).
 """
 from __future__ import annotations
 
