@@ -47,9 +47,15 @@ def _peaks():
 
 
 def _csrc_digest() -> str:
-    """digest of the CUDA sources and build flags (the one paper_2607_08743_b200/build.py stamps the library with)"""
+    """digest of the kernel sources (csrc/*, include/sacra.h) and of the nvcc flags"""
+    import hashlib
     from paper_2607_08743_b200 import build as b
-    return b._digest()
+    h = hashlib.sha256(" ".join(b.FLAGS).encode())
+    files = [os.path.join(ROOT, "include", "sacra.h")] + [os.path.join(b.CSRC, f) for f in os.listdir(b.CSRC)]
+    for f in sorted(files):
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
 
 
 def _committed_traffic(workload: str):
