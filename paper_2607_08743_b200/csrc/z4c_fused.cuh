@@ -78,12 +78,15 @@ __device__ __forceinline__ void z4c_point(const Src& src, const Params& P, const
   {
     const double gxx = g[0], gxy = g[1], gxz = g[2], gyy = g[3], gyz = g[4], gzz = g[5];
     const double det = (gxx * (gyy * gzz - gyz * gyz) - gxy * (gxy * gzz - gyz * gxz)) + gxz * (gxy * gyz - gyy * gxz);
-    gi[0] = (gyy * gzz - gyz * gyz) / det;
-    gi[1] = (gxz * gyz - gxy * gzz) / det;
-    gi[2] = (gxy * gyz - gxz * gyy) / det;
-    gi[3] = (gxx * gzz - gxz * gxz) / det;
-    gi[4] = (gxy * gxz - gxx * gyz) / det;
-    gi[5] = (gxx * gyy - gxy * gxy) / det;
+    // one IEEE division, six products: gt^ij feeds only the relaxed fields (K-hat, Theta, At_ij, Gt^i, B^i), where a last-bit
+    // difference from the oracle's six divisions is far inside the tolerance
+    const double rdet = 1.0 / det;
+    gi[0] = (gyy * gzz - gyz * gyz) * rdet;
+    gi[1] = (gxz * gyz - gxy * gzz) * rdet;
+    gi[2] = (gxy * gyz - gxz * gyy) * rdet;
+    gi[3] = (gxx * gzz - gxz * gxz) * rdet;
+    gi[4] = (gxy * gxz - gxx * gyz) * rdet;
+    gi[5] = (gxx * gyy - gxy * gxy) * rdet;
   }
   const double K = Kh + 2.0 * Th;                                        // item 7: K = K-hat + 2 Theta
 
