@@ -549,11 +549,13 @@ struct LinComb {
   const double* u[3];
   double w[3];
   int n;
+  int lo[3], hi[3];   // storage-index box [lo, hi) per axis (x, y, z) the combination is formed on
 };
 __global__ void __launch_bounds__(256) k_lincomb(const __grid_constant__ DevPatch p, const __grid_constant__ LinComb L,
                                                  double* __restrict__ out) {
-  const int sx = p.nx + 2 * NG, sy = p.ny + 2 * NG;
-  const long long c0 = p.offset + (long long)blockIdx.y * p.fstride + (long long)blockIdx.x * p.sz;
+  const int sx = L.hi[0] - L.lo[0], sy = L.hi[1] - L.lo[1];
+  const long long c0 = p.offset + (long long)blockIdx.y * p.fstride + (long long)(L.lo[2] + (int)blockIdx.x) * p.sz +
+                       (long long)L.lo[1] * p.pitch + L.lo[0];
   for (int q = threadIdx.x; q < sx * sy; q += blockDim.x) {
     const long long c = c0 + (long long)(q / sx) * p.pitch + (q % sx);
     double s = L.w[0] * L.u[0][c] + L.w[1] * L.u[1][c];
@@ -1105,13 +1107,19 @@ int sacra_time_weights(int nlevels, double theta, double* w) {
   return SACRA_OK;
 }
 
+// box: storage-index bounds [lo, hi) per axis, or nullptr for the whole storage of the patch
 static int launch_lincomb(const sacra_patch_t* p, int n, const double* u0, const double* u1, const double* u2,
-                          const double* w, double* out, cudaStream_t st) {
+                          const double* w, double* out, cudaStream_t st, const int* lo = nullptr, const int* hi = nullptr) {
   LinComb L;
   L.u[0] = u0; L.u[1] = u1; L.u[2] = n == 3 ? u2 : u0;
   L.w[0] = w[0]; L.w[1] = w[1]; L.w[2] = n == 3 ? w[2] : 0.0;
   L.n = n;
-  k_lincomb<<<dim3(p->nz + 2 * NG, NF), 256, 0, st>>>(to_dev(*p), L, out);
+  const int s[3] = {p->nx + 2 * NG, p->ny + 2 * NG, p->nz + 2 * NG};
+  for (int a = 0; a < 3; ++a) {
+    L.lo[a] = lo ? (lo[a] < 0 ? 0 : lo[a]) : 0;
+    L.hi[a] = hi ? (hi[a] > s[a] ? s[a] : hi[a]) : s[a];
+  }
+  k_lincomb<<<dim3(L.hi[2] - L.lo[2], NF), 256, 0, st>>>(to_dev(*p), L, out);
   return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
 }
 
@@ -1168,13 +1176,21 @@ int sacra_subcycle_step(const sacra_patch_t* parent, const sacra_patch_t* child,
     k_prolong_ghosts<<<dim3((nshell + 127) / 128, NF), 128, 0, st>>>(L, up, uc);
     return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
   };
+  // the prolongation reads the parent's active cells org - 5 .. org + n_child / 2 + 3 per axis: the time
+  // interpolation is formed on that box only, not on the whole parent
+  int blo[3], bhi[3];
+  const int ncs[3] = {child->nx, child->ny, child->nz};
+  for (int a = 0; a < 3; ++a) {
+    blo[a] = org[a] - 5 + NG;
+    bhi[a] = org[a] + ncs[a] / 2 + 3 + NG + 1;
+  }
   for (int m = 0; m < 2; ++m) {
     const double* in[4] = {u_child, w0, w1, w0};
     double* out[4] = {w0, w1, w0, u_child};
     for (int s = 0; s < 4; ++s) {
       double w[3];
       sacra_time_weights(nlev, ((double)m + cs[s]) / 2.0, w);
-      if ((e = launch_lincomb(parent, nlev, lev[0], lev[1], lev[2], w, tmp, st))) return e;
+      if ((e = launch_lincomb(parent, nlev, lev[0], lev[1], lev[2], w, tmp, st, blo, bhi))) return e;
       if ((e = prolong(tmp, const_cast<double*>(in[s])))) return e;
       if ((e = launch_z4c(child, 1, prm, s + 1, in[s], nullptr, u_child, out[s], acc, st))) return e;
     }

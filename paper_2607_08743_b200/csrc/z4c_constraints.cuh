@@ -42,17 +42,18 @@ __device__ __forceinline__ void constraints_point(const Src& src, const GridCoef
   {
     const double gxx = g[0], gxy = g[1], gxz = g[2], gyy = g[3], gyz = g[4], gzz = g[5];
     const double det = (gxx * (gyy * gzz - gyz * gyz) - gxy * (gxy * gzz - gyz * gxz)) + gxz * (gxy * gyz - gyy * gxz);
-    gi[0] = (gyy * gzz - gyz * gyz) / det;
-    gi[1] = (gxz * gyz - gxy * gzz) / det;
-    gi[2] = (gxy * gyz - gxz * gyy) / det;
-    gi[3] = (gxx * gzz - gxz * gxz) / det;
-    gi[4] = (gxy * gxz - gxx * gyz) / det;
-    gi[5] = (gxx * gyy - gxy * gxy) / det;
+    const double rdet = 1.0 / det;
+    gi[0] = (gyy * gzz - gyz * gyz) * rdet;
+    gi[1] = (gxz * gyz - gxy * gzz) * rdet;
+    gi[2] = (gxy * gyz - gxz * gyy) * rdet;
+    gi[3] = (gxx * gzz - gxz * gxz) * rdet;
+    gi[4] = (gxy * gxz - gxx * gyz) * rdet;
+    gi[5] = (gxx * gyy - gxy * gxy) * rdet;
   }
   const double K = Kh + 2.0 * Th;
   double B[6];
 #pragma unroll
-  for (int n = 0; n < 6; ++n) B[n] = A[n] + g[n] * K / 3.0;
+  for (int n = 0; n < 6; ++n) B[n] = fma(g[n], K * (1.0 / 3.0), A[n]);
 
   // ---- derivatives, field by field; second derivatives of gt_ij and the gradient of B_ij are folded at once -------
   // the derivatives that are only needed at the very end (d_k W, d_i d_j W, d_k gt_ij) wait in the Tensor Memory
@@ -103,7 +104,7 @@ __device__ __forceinline__ void constraints_point(const Src& src, const GridCoef
     field_derivs<true, false, false>(src.template field<F_A + N>(), pc, S);                         \
     wait_ld(dgn);                                                                                   \
     double dBn[3];                                                                                  \
-    _Pragma("unroll") for (int k = 0; k < 3; ++k) dBn[k] = S.d1[k] + (dgn.get(k) * K + g[N] * dK[k]) / 3.0; \
+    _Pragma("unroll") for (int k = 0; k < 3; ++k) dBn[k] = fma(fma(dgn.get(k), K, g[N] * dK[k]), 1.0 / 3.0, S.d1[k]); \
     const double va = (gi[sym(0, A)] * dBn[0] + gi[sym(1, A)] * dBn[1]) + gi[sym(2, A)] * dBn[2];   \
     const double vb = (gi[sym(0, Bx)] * dBn[0] + gi[sym(1, Bx)] * dBn[1]) + gi[sym(2, Bx)] * dBn[2]; \
     _Pragma("unroll") for (int i = 0; i < 3; ++i)                                                   \
@@ -219,7 +220,7 @@ __device__ __forceinline__ void constraints_point(const Src& src, const GridCoef
   // ---- momentum constraint ------------------------------------------------------------------------------------------
   double w[3], wu[3];                 // w_j = d_j W / W, w^c = gt^cd w_d
 #pragma unroll
-  for (int j = 0; j < 3; ++j) w[j] = dW[j] / W;
+  for (int j = 0; j < 3; ++j) w[j] = dW[j] * (1.0 / W);
 #pragma unroll
   for (int c = 0; c < 3; ++c) wu[c] = (gi[sym(c, 0)] * w[0] + gi[sym(c, 1)] * w[1]) + gi[sym(c, 2)] * w[2];
   // full connection Gamma^c_ja = Gt^c_ja + C^c_ja ,  C^c_ja = -( delta^c_j w_a + delta^c_a w_j - gt_ja w^c ), formed once;
