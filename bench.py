@@ -30,11 +30,11 @@ NF = 25
 # Algorithmic work per point: 16 field passes x 8 B x 25 fields per RK4 step (the
 # minimum of any RK4 formulation, 3 + 5 + 5 + 3; the increment-form acc of this library moves 3 + 5 + 5 + 4 = 17 with
 # SACRA_FLAG_SKIP_INCREMENT, which the timed steps set, and 18 without), i.e. 800 B per substage launch on average;
-# FP64 work per RHS evaluation + RK update after CSE: 3 227 FP64 instructions (DADD 1 399, DMUL 815, DFMA 1 013 per
-# point in the SASS of k_z4c<2>, profiles/r02_sass_histogram.md) = 4 240 flop with FMA = 2.
+# FP64 work per RHS evaluation + RK update after CSE: 3 206 FP64 instructions (DADD 1 399, DMUL 818, DFMA 989 per
+# point in the SASS of k_z4c<2>, profiles/r02_sass_histogram.md) = 4 195 flop with FMA = 2.
 ALG_BYTES_PER_POINT_STEP = 16 * 8 * NF
-ALG_FLOP_PER_POINT_STAGE = 4240.0
-ALG_FP64_INSTR_PER_POINT_STAGE = 3227.0
+ALG_FLOP_PER_POINT_STAGE = 4195.0
+ALG_FP64_INSTR_PER_POINT_STAGE = 3206.0
 FP64_LANES_PER_SM, N_SM = 64, 148
 
 
