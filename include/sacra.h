@@ -234,6 +234,17 @@ int sacra_subcycle_step(const sacra_patch_t* parent, const sacra_patch_t* child,
  *                        face is what its high neighbour unpacks at its low face, and vice versa.
  * The transfer itself is the caller's (paper_2607_08743_b200/halo.py: torch.distributed point-to-point over NCCL). */
 int64_t sacra_face_doubles(const sacra_patch_t* p, int axis);
+/* Overlap of the exchange with the computation (PAPER.md:378 lists it as future work): sacra_rk4_substep in two parts.
+ * exchange_faces: HOST int32_t[6] (x- x+ y- y+ z- z+), non-zero where the ghosts behind the face come from an exchange.
+ *   SACRA_PART_INTERIOR  the active cells more than 3 cells away from every flagged face: they read no exchanged ghost
+ *                        cell, so this part can run while the messages are in flight;
+ *   SACRA_PART_SHELL     the other active cells, after the unpack (tiles without such a cell are skipped).
+ * The two parts write disjoint cells; together they give sacra_rk4_substep bit for bit. Same argument rules. */
+#define SACRA_PART_INTERIOR 1
+#define SACRA_PART_SHELL 2
+int sacra_rk4_substep_part(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, int stage, int part,
+                           const int32_t* exchange_faces, const double* u_n, const double* u_in, double* u_out, double* acc,
+                           void* cuda_stream);
 int sacra_pack_face(const sacra_patch_t* p, const double* u, int axis, int side, double* buf, void* cuda_stream);
 int sacra_unpack_face(const sacra_patch_t* p, double* u, int axis, int side, const double* buf, void* cuda_stream);
 

@@ -27,11 +27,15 @@ struct DevPatch {
   double dx, dt;
   GridCoef gc;             // 1/(12 h) ... of the derivative stage (launch_z4c fills in the KO factor)
   unsigned shell;          // bit 2a + side: that face is a Sommerfeld face (its 3 outermost layers are the boundary shell)
+  unsigned xshell;         // bit 2a + side: ghosts behind that face come from a halo exchange (partial launches, below)
 };
 struct PatchBatch {
   DevPatch p[MAXP];
   int first_block[MAXP + 1];   // prefix sum of blocks per patch (block -> patch lookup)
   int np;
+  // 0: every active cell. Partial launches for the overlap of the halo exchange with the computation: 1 = the cells
+  // that need no exchanged ghost (more than 3 cells from every xshell face), 2 = the others, tiles without any skipped
+  int part;
 };
 
 // ---------------------------------------------------------------------------------------------------
@@ -137,10 +141,15 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(const __grid_constant__ Pat
 struct ShellGeom {
   double origin[MAXP][3];
 };
-__device__ __forceinline__ bool in_shell(const DevPatch& p, int i, int j, int k) {
-  const unsigned s = p.shell;
+__device__ __forceinline__ bool in_shell(unsigned s, const DevPatch& p, int i, int j, int k) {
   return ((s & 1u) && i < NG) || ((s & 2u) && i >= p.nx - NG) || ((s & 4u) && j < NG) || ((s & 8u) && j >= p.ny - NG) ||
          ((s & 16u) && k < NG) || ((s & 32u) && k >= p.nz - NG);
+}
+// does the tile [x0, x0 + tx) x [y0, y0 + ty) x [z0, z0 + tz) hold a cell within NG cells of a flagged exchange face?
+__device__ __forceinline__ bool tile_touches_xshell(const DevPatch& p, int x0, int y0, int z0, int tx, int ty, int tz) {
+  const unsigned s = p.xshell;
+  return ((s & 1u) && x0 < NG) || ((s & 2u) && x0 + tx > p.nx - NG) || ((s & 4u) && y0 < NG) || ((s & 8u) && y0 + ty > p.ny - NG) ||
+         ((s & 16u) && z0 < NG) || ((s & 32u) && z0 + tz > p.nz - NG);
 }
 // first derivative along a stride at index i of an axis whose usable index range is [lo, hi]
 __device__ __forceinline__ double d1_bounded(const double* u, long long st, int i, int lo, int hi, double inv12h) {
@@ -171,7 +180,7 @@ __global__ void __launch_bounds__(256) k_sommerfeld(const __grid_constant__ Patc
   const double z = G.origin[ip][2] + (double)k * h;
   for (int q = threadIdx.x; q < p.nx * p.ny; q += blockDim.x) {
     const int i = q % p.nx, j = q / p.nx;
-    if (!in_shell(p, i, j, k)) continue;
+    if (!in_shell(p.shell, p, i, j, k)) continue;
     const long long c = fo + (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
     const double* uc = u_in + c;
     const double x = G.origin[ip][0] + (double)i * h, y = G.origin[ip][1] + (double)j * h;
@@ -316,27 +325,44 @@ __global__ void __launch_bounds__(Tile::NTH, 1) k_z4c(const __grid_constant__ Pa
   using C = Tile;
   using Src = TileSource<C, rk_mode(EPI < 0 ? 0 : EPI), std::conditional_t<EPI < 0, ConStream, Z4cStream>>;
   const int ntiles = B.first_block[B.np];
-  int t = blockIdx.x;
-  if (t >= ntiles) return;
+  if ((int)blockIdx.x >= ntiles) return;
+  // the CTA's tiles: blockIdx.x, + gridDim.x, ...; a shell-only launch (B.part == 2) skips the tiles without a shell cell
+  auto selected = [&](int tt) {
+    if (B.part != 2) return true;
+    const TileId q = locate_inl<C>(B, tt);
+    const DevPatch& pq = B.p[q.ip];
+    return tile_touches_xshell(pq, q.bx * C::TX, q.by * C::TY, q.bz * C::TZ, C::TX, C::TY, C::TZ);
+  };
+  auto advance = [&](int tt) {
+    do tt += (int)gridDim.x;
+    while (tt < ntiles && !selected(tt));
+    return tt;
+  };
   // 1-D block of NT compute threads (thread q = point (q % TX, q / TX % TY, q / (TX TY)) of the tile) + one producer warp
   const int tid = threadIdx.x;
   TileId* desc = Src::desc();
   uint32_t* tm_base = reinterpret_cast<uint32_t*>(tile_smem + C::TMB_OFF);
   static_assert(sizeof(TileId) == 16, "descriptor slots");
   if (tid == 0) {
-    desc[0] = locate_inl<C>(B, t);
+    int t0 = blockIdx.x;
+    if (!selected(t0)) t0 = advance(t0);
+    tm_base[1] = (uint32_t)t0;
+    if (t0 < ntiles) desc[0] = locate_inl<C>(B, t0);
     Src::init_barriers();
   }
   if (tid < 32) tmem::alloc_all(tm_base);   // warp 0 owns the allocation (and frees it at the end)
   tmem::fence_before_sync();
   __syncthreads();
   tmem::fence_after_sync();
+  const int t = (int)tm_base[1];   // the CTA's first tile
   // The kernel starts with 65536 / NTH = 128 registers per thread; the producer warpgroup hands its registers to the
   // compute warpgroups (a kernel that uses setmaxnreg must not contain calls: locate_inl)
-  if (tid >= C::NT) {
+  if (t >= ntiles) {
+    // nothing to do for this CTA (partial launch)
+  } else if (tid >= C::NT) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::REG_PRODUCER));
     if (tid % 32 == 0 && tid < C::NT + 96)
-      Src::producer((tid - C::NT) / 32, &M, t, (int)gridDim.x, ntiles, [&](int tt) { return locate_inl<C>(B, tt); });
+      Src::producer((tid - C::NT) / 32, &M, t, ntiles, [&](int tt) { return locate_inl<C>(B, tt); }, advance);
   } else {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::REG_COMPUTE));
     const int tx = tid % C::TX, ty = tid / C::TX % C::TY, tz = tid / (C::TX * C::TY);
@@ -356,20 +382,19 @@ __global__ void __launch_bounds__(Tile::NTH, 1) k_z4c(const __grid_constant__ Pa
 #pragma unroll 1
     for (uint32_t iter = 0;; ++iter) {
       const DevPatch& p = B.p[id.ip];
-      const int tn = t + gridDim.x;
-      src.has_next = tn < ntiles;
       src.iter = iter;
       const int i = id.bx * C::TX + tx, j = id.by * C::TY + ty, k = id.bz * C::TZ + tz;
-      // cells of the Sommerfeld boundary shell belong to k_sommerfeld
-      const bool active = (i < p.nx) & (j < p.ny) & (k < p.nz) && !(p.shell && in_shell(p, i, j, k));
+      // cells of the Sommerfeld boundary shell belong to k_sommerfeld; a partial launch takes the cells inside / outside
+      // the exchange shell only
+      bool active = (i < p.nx) & (j < p.ny) & (k < p.nz) && !(p.shell && in_shell(p.shell, p, i, j, k));
+      if (B.part) active = active && (in_shell(p.xshell, p, i, j, k) == (B.part == 2));
       const long long c = (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
       Emitter<(EPI < 0 ? 0 : EPI), Src> emit{src, rhs, rk.u_out, rk.acc, p.offset + c, p.fstride, p.dt, active};
       src.begin_tile();
       if constexpr (EPI < 0) constraints_point(src, p.gc, emit);
       else z4c_point(src, P, p.gc, emit);
-      if (!src.has_next) break;
-      t = tn;
-      id = desc[(iter + 1) & 1u];   // written by the producer at the top of this tile
+      id = desc[(iter + 1) & 1u];   // written by the producer at the top of this tile; ip < 0: no more tiles
+      if (id.ip < 0) break;
     }
   }
   tmem::fence_before_sync();
@@ -608,6 +633,7 @@ static DevPatch to_dev(const sacra_patch_t& a) {
   d.pitch = a.pitch_x; d.sz = a.pitch_x * (long long)(a.ny + 2 * NG);
   d.fstride = a.field_stride; d.offset = a.patch_offset; d.dx = a.dx; d.dt = a.dt;
   d.shell = 0;
+  d.xshell = 0;
   d.gc = grid_coef(a.dx, 0.0);
   return d;
 }
@@ -624,6 +650,7 @@ static int launch_fill(const sacra_patch_t* p, int npatch, double* u, cudaStream
                        const sacra_boundary_t* bnd = nullptr) {
   for (int q0 = 0; q0 < npatch; q0 += MAXP) {
     PatchBatch B;
+    B.part = 0;
     FillModes M;
     B.np = (npatch - q0 < MAXP) ? npatch - q0 : MAXP;
     int nb = 0, split = 1;
@@ -670,6 +697,7 @@ static int launch_sommerfeld(const sacra_patch_t* p, int npatch, const sacra_bou
   RkArgs rk{u_n, u_out, acc};
   for (int q0 = 0; q0 < npatch; q0 += MAXP) {
     PatchBatch B;
+    B.part = 0;
     ShellGeom G;
     B.np = (npatch - q0 < MAXP) ? npatch - q0 : MAXP;
     int nb = 0;
@@ -789,13 +817,14 @@ static cudaError_t launch_one(int grid, cudaStream_t st, const PatchBatch& B, co
 
 static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, int epi,
                       const double* u_in, double* rhs, const double* u_n, double* u_out, double* acc,
-                      cudaStream_t st, const sacra_boundary_t* bnd = nullptr) {
+                      cudaStream_t st, const sacra_boundary_t* bnd = nullptr, int part = 0, unsigned xfaces = 0) {
   const Params P = to_dev(*prm);
   RkArgs rk{u_n, u_out, acc};
   const int sms = num_sms();
   if (sms <= 0) return SACRA_ERR_CUDA;
   for (int q0 = 0; q0 < npatch; q0 += MAXP) {
     PatchBatch B;
+    B.part = 0;
     TileMaps M;
     B.np = (npatch - q0 < MAXP) ? npatch - q0 : MAXP;
     int nb = 0;
@@ -804,6 +833,7 @@ static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* 
       B.p[q] = to_dev(a);
       B.p[q].gc = grid_coef(a.dx, prm->ko_sigma);
       if (bnd) B.p[q].shell = shell_bits(bnd[q0 + q]);
+      B.p[q].xshell = xfaces;
       B.first_block[q] = nb;
       nb += ((a.nx + Tile::TX - 1) / Tile::TX) * ((a.ny + Tile::TY - 1) / Tile::TY) * ((a.nz + Tile::TZ - 1) / Tile::TZ);
       if (int e = cached_map(a, u_in, Tile::PX, Tile::PY, Tile::PZ, 1, &M.box[q])) return e;
@@ -814,6 +844,7 @@ static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* 
       }
     }
     B.first_block[B.np] = nb;
+    B.part = part;
     const int grid = nb < sms ? nb : sms;   // persistent CTAs (one per SM: the kernel owns the SM's Tensor Memory)
     cudaError_t err;
     switch (epi) {
@@ -878,6 +909,27 @@ int sacra_rk4_substep(const sacra_patch_t* p, int npatch, const sacra_params_t* 
   if (u_n != u_out && overlap(u_n, ext, u_out, ext)) return SACRA_ERR_BADARG;
   const int epi = (stage == 4 && (prm->flags & SACRA_FLAG_SKIP_INCREMENT)) ? 5 : stage;
   return launch_z4c(p, npatch, prm, epi, u_in, nullptr, u_n, u_out, acc, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int sacra_rk4_substep_part(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, int stage, int part,
+                           const int32_t* exchange_faces, const double* u_n, const double* u_in, double* u_out, double* acc,
+                           void* cuda_stream) {
+  if (!p || !prm || !exchange_faces || !u_n || !u_in || !u_out || !acc) return SACRA_ERR_NULL;
+  if (int e = check_patches(p, npatch)) return e;
+  if (stage < 1 || stage > 4 || (part != SACRA_PART_INTERIOR && part != SACRA_PART_SHELL)) return SACRA_ERR_BADARG;
+  if (!aligned16(u_n) || !aligned16(u_in) || !aligned16(u_out) || !aligned16(acc)) return SACRA_ERR_ALIGN;
+  const long long ext = state_extent(p, npatch);
+  if (stage == 1 && u_n != u_in) return SACRA_ERR_BADARG;
+  if (overlap(u_out, ext, u_in, ext)) return SACRA_ERR_BADARG;
+  if (overlap(acc, ext, u_in, ext) || overlap(acc, ext, u_n, ext) || overlap(acc, ext, u_out, ext)) return SACRA_ERR_BADARG;
+  if (u_n != u_in && overlap(u_n, ext, u_in, ext)) return SACRA_ERR_BADARG;
+  if (u_n != u_out && overlap(u_n, ext, u_out, ext)) return SACRA_ERR_BADARG;
+  unsigned faces = 0;
+  for (int a = 0; a < 6; ++a)
+    if (exchange_faces[a]) faces |= 1u << a;
+  const int epi = (stage == 4 && (prm->flags & SACRA_FLAG_SKIP_INCREMENT)) ? 5 : stage;
+  return launch_z4c(p, npatch, prm, epi, u_in, nullptr, u_n, u_out, acc, static_cast<cudaStream_t>(cuda_stream), nullptr, part,
+                    faces);
 }
 
 int sacra_rk4_step(const sacra_patch_t* p, int npatch, const sacra_params_t* prm, double* u, double* work,
@@ -1000,6 +1052,7 @@ int sacra_constraint_norms(const sacra_patch_t* p, int npatch, const double* con
   int planes = 0;
   for (int q0 = 0; q0 < npatch; q0 += MAXP) {
     PatchBatch B;
+    B.part = 0;
     B.np = (npatch - q0 < MAXP) ? npatch - q0 : MAXP;
     int nb = 0;
     for (int q = 0; q < B.np; ++q) {

@@ -300,7 +300,6 @@ struct TileSource {
   uint32_t tm;             // Tensor Memory: address of double 0 of this thread's strip (a double = 2 columns)
   int ey, ez;              // shared memory: this thread's entries of the e arrays
   int xh, yh;              // halo duties of the e exchange (TileLoader)
-  bool has_next;
   uint32_t iter;           // tiles done by this CTA (ring phases)
 
   __device__ __forceinline__ static uint64_t* bar(int i) { return reinterpret_cast<uint64_t*>(tile_smem + C::BAR_OFF) + i; }
@@ -383,15 +382,21 @@ struct TileSource {
   // desc()[(it + 1) & 1] is written at the top of tile `it`, when every compute warp is inside tile it - 1 or later (it
   // read that entry at the end of tile it - 2); the compute warps read it at the end of tile `it`, after many waits
   // on "full" barriers armed later than the write.
-  template <class Locate>
-  __device__ __forceinline__ static void producer(int role, const TileMaps* maps, int t, int stride, int ntiles,
-                                                  Locate locate) {
+  // `advance(t)`: the CTA's next tile after t (t + gridDim.x, or further when a partial launch skips tiles), >= ntiles
+  // if there is none. Role 0 always publishes the next descriptor, with ip = -1 for "no more tiles": that is how the
+  // compute warps learn that they are done.
+  template <class Locate, class Advance>
+  __device__ __forceinline__ static void producer(int role, const TileMaps* maps, int t, int ntiles, Locate locate,
+                                                  Advance advance) {
     if (RK != 2 && role != 0) return;
     uint32_t it = 0;
     TileId cur = desc()[0], nxt = cur;
-    bool has_next = t + stride < ntiles;
+    int tn = advance(t);
+    bool has_next = tn < ntiles;
     if (role == 0) {
-      if (has_next) desc()[1] = nxt = locate(t + stride);
+      if (has_next) nxt = locate(tn);
+      else nxt.ip = -1;
+      desc()[1] = nxt;
       issue_centre(maps, cur);
 #pragma unroll 1
       for (int S = 0; S < C::NS - 1; ++S) issue_box(maps, it, S, cur);
@@ -410,11 +415,14 @@ struct TileSource {
           else if (has_next) issue_box(maps, it, S, nxt);
         }
         if (!has_next) break;
-        t += stride;
+        t = tn;
         ++it;
         cur = nxt;
-        has_next = t + stride < ntiles;
-        if (has_next) desc()[(it + 1u) & 1u] = nxt = locate(t + stride);
+        tn = advance(t);
+        has_next = tn < ntiles;
+        if (has_next) nxt = locate(tn);
+        else nxt.ip = -1;
+        desc()[(it + 1u) & 1u] = nxt;
       }
     } else {
       const CUtensorMap* map = role == 1 ? maps->un : maps->acc;
@@ -427,9 +435,10 @@ struct TileSource {
           issue_rk(map, role - 1, q, e, cur);
         }
         if (!has_next) break;
-        t += stride;
+        t = tn;
         cur = locate(t);
-        has_next = t + stride < ntiles;
+        tn = advance(t);
+        has_next = tn < ntiles;
       }
     }
   }

@@ -103,15 +103,39 @@ def exchange_halos(patch, u, topo: CartTopology, rank: int, ops=None, group=None
     return sent
 
 
-def rk4_step_distributed(patch, params, u, work, topo: CartTopology, rank: int, ops=None, group=None, buffers=None):
+def rk4_step_distributed(patch, params, u, work, topo: CartTopology, rank: int, ops=None, group=None, buffers=None,
+                         overlap=False):
     """One RK4 step of this rank's block: the halo exchange stands where sacra_rk4_step has its periodic fill
-    (exchange, substage, four times; exchange of the result). work: 3 states like sacra_rk4_step."""
+    (exchange, substage, four times; exchange of the result). work: 3 states like sacra_rk4_step.
+
+    overlap=True (PAPER.md:378 lists it as future work): per substage the cells that need no exchanged ghost
+    (sacra_rk4_substep_part, PART_INTERIOR) are computed on the caller's stream WHILE the stage input's halos are packed,
+    sent and unpacked on a second stream; the boundary shell (PART_SHELL) follows when both are done. Same bits."""
     from . import sacra
     n = u.numel()
     w0, w1, acc = work[:n], work[n:2 * n], work[2 * n:]
     buffers = buffers if buffers is not None else {}
     seq = [(u, w0), (w0, w1), (w1, w0), (w0, u)]
+    if not overlap:
+        for stage, (src, dst) in enumerate(seq, start=1):
+            exchange_halos(patch, src, topo, rank, ops, group, buffers)
+            sacra.rk4_substep([patch], params, stage, u, src, dst, acc)
+        exchange_halos(patch, u, topo, rank, ops, group, buffers)
+        return
+    import torch
+    main = torch.cuda.current_stream()
+    if "comm_stream" not in buffers:
+        buffers["comm_stream"] = torch.cuda.Stream()
+    comm = buffers["comm_stream"]
+    faces = [1] * 6                      # every face of a block of a periodic decomposition is an exchange face
+    cops = ops or CudaOps()
     for stage, (src, dst) in enumerate(seq, start=1):
-        exchange_halos(patch, src, topo, rank, ops, group, buffers)
-        sacra.rk4_substep([patch], params, stage, u, src, dst, acc)
-    exchange_halos(patch, u, topo, rank, ops, group, buffers)
+        comm.wait_stream(main)           # the stage input is complete
+        with torch.cuda.stream(comm):
+            cops.stream = comm
+            exchange_halos(patch, src, topo, rank, cops, group, buffers)
+        sacra.rk4_substep_part([patch], params, stage, sacra.PART_INTERIOR, faces, u, src, dst, acc)
+        main.wait_stream(comm)           # ghosts of the stage input are in place
+        sacra.rk4_substep_part([patch], params, stage, sacra.PART_SHELL, faces, u, src, dst, acc)
+    cops.stream = None
+    exchange_halos(patch, u, topo, rank, cops, group, buffers)

@@ -24,7 +24,7 @@ EXPORTS = ("sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4
            "sacra_fill_ghosts_bc", "sacra_restrict", "sacra_prolong_ghosts",
            "sacra_fill_ghosts_faces", "sacra_sommerfeld_rhs", "sacra_rk4_substep_bc", "sacra_rk4_step_bc",
            "sacra_time_weights", "sacra_lincomb", "sacra_subcycle_step",
-           "sacra_face_doubles", "sacra_pack_face", "sacra_unpack_face")
+           "sacra_face_doubles", "sacra_pack_face", "sacra_unpack_face", "sacra_rk4_substep_part")
 
 
 class SacraPatch(C.Structure):
@@ -79,7 +79,8 @@ def _load():
     lib.sacra_face_doubles.restype = C.c_int64
     lib.sacra_pack_face.argtypes = [vp, dp, i32, i32, dp, vp]
     lib.sacra_unpack_face.argtypes = [vp, dp, i32, i32, dp, vp]
-    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:19] + EXPORTS[20:22]:
+    lib.sacra_rk4_substep_part.argtypes = [vp, i32, vp, i32, i32, vp, dp, dp, dp, dp, vp]
+    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:19] + EXPORTS[20:23]:
         getattr(lib, n).restype = C.c_int
     lib.sacra_strerror.argtypes = [C.c_int]
     lib.sacra_strerror.restype = C.c_char_p
@@ -294,3 +295,15 @@ def pack_face(patch, u, axis, side, buf, stream=None):
 def unpack_face(patch, u, axis, side, buf, stream=None):
     """the 3 ghost layers behind a face <- buf (sacra_unpack_face)"""
     _check(lib.sacra_unpack_face(_one(patch), _ptr(u), int(axis), int(side), _ptr(buf), _stream(stream)))
+
+
+PART_INTERIOR, PART_SHELL = 1, 2
+
+
+def rk4_substep_part(patches, params, stage, part, exchange_faces, u_n, u_in, u_out, acc, stream=None):
+    """sacra_rk4_substep on the cells that need no exchanged ghost (PART_INTERIOR) or on the others (PART_SHELL)"""
+    ps = make_patches(patches) if patches is not None else None
+    pr = make_params(params) if params is not None else None
+    xf = (C.c_int32 * 6)(*[int(v) for v in exchange_faces]) if exchange_faces is not None else None
+    _check(lib.sacra_rk4_substep_part(ps, len(ps) if ps is not None else 0, _ref(pr), int(stage), int(part), xf,
+                                      _ptr(u_n), _ptr(u_in), _ptr(u_out), _ptr(acc), _stream(stream)))

@@ -197,3 +197,19 @@ def test_subcycling_argument_checks():
     assert call(pp[0], pc[0], ok, bufs[0], None, *bufs[2:]) == sacra.ERR_NULL
     assert _code(sacra.lincomb, pp[0], [FAKE, FAKE + step], [0.5, 0.5], FAKE + 64) == sacra.ERR_BADARG
     assert _code(sacra.lincomb, pp[0], [FAKE, None], [0.5, 0.5], FAKE + 2 * step) == sacra.ERR_NULL
+
+
+def test_partial_substep_and_face_buffer_argument_checks():
+    ps, total = _patch()
+    far = lambda k: FAKE + 8 * k * (total + 64)
+    ok = [1] * 6
+    assert _code(sacra.rk4_substep_part, ps, PRM, 2, 3, ok, FAKE, far(1), far(2), far(3)) == sacra.ERR_BADARG     # unknown part
+    assert _code(sacra.rk4_substep_part, ps, PRM, 5, 1, ok, FAKE, far(1), far(2), far(3)) == sacra.ERR_BADARG
+    assert _code(sacra.rk4_substep_part, ps, PRM, 1, 1, ok, far(1), FAKE, far(2), far(3)) == sacra.ERR_BADARG     # stage 1: u_n is u_in
+    assert _code(sacra.rk4_substep_part, ps, PRM, 2, 2, None, FAKE, far(1), far(2), far(3)) == sacra.ERR_NULL
+    assert _code(sacra.rk4_substep_part, ps, PRM, 2, 2, ok, FAKE, far(1), far(1) + 64, far(3)) == sacra.ERR_BADARG
+    assert sacra.face_doubles(ps[0], 0) == 25 * 3 * 14 * 14
+    assert _code(sacra.pack_face, ps[0], FAKE, 3, 0, far(1)) == sacra.ERR_BADARG
+    assert _code(sacra.pack_face, ps[0], FAKE, 0, 2, far(1)) == sacra.ERR_BADARG
+    assert _code(sacra.unpack_face, ps[0], FAKE, 0, 0, FAKE + 64) == sacra.ERR_BADARG                             # buffer inside the state
+    assert _code(sacra.unpack_face, ps[0], None, 0, 0, far(1)) == sacra.ERR_NULL

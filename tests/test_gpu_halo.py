@@ -56,3 +56,65 @@ def test_single_rank_exchange_equals_periodic_fill_and_step():
     halo.rk4_step_distributed(p, w.params, u, wu, topo, 0)
     sacra.rk4_step([p], w.params, v, wv)
     assert np.array_equal(host(u), host(v)) and np.array_equal(host(wu[2 * n:]), host(wv[2 * n:]))
+
+
+def _smooth(w):
+    for ip, p in enumerate(w.patches):
+        for f in range(NF):
+            a = w.active_view(w.state, ip, f)
+            a *= 0.01
+            if f in (wl.F_W, wl.F_G, wl.F_G + 3, wl.F_G + 5, wl.F_ALP):
+                a += 1.0
+    return w
+
+
+@pytest.mark.parametrize("faces", [[1] * 6, [1, 0, 0, 1, 1, 0], [0, 0, 0, 0, 1, 1]])
+def test_interior_plus_shell_equals_the_whole_substep_bitwise(faces):
+    """sacra_rk4_substep_part: the two parts write disjoint cells and together are sacra_rk4_substep, all four stages
+    (acc is read-modify-write), on a ragged batch with patches smaller than the shell and tiles that are skipped"""
+    dims = [(40, 21, 26), (6, 6, 6), (17, 9, 50)]
+    rng = np.random.default_rng(6)
+    ps, total = wl.make_layout(dims, [0.1, 0.2, 0.15], [0.025, 0.05, 0.03], [(0, 0, 0)] * 3)
+    w = _smooth(wl.Workload("part", ps, dict(wl.DEFAULT_PARAMS), rng.normal(size=total)))
+    un = dev(w.state)
+    sacra.fill_ghosts(ps, un)
+    uin = un
+    acc_a = torch.zeros(total, dtype=torch.float64, device="cuda")
+    acc_b = torch.zeros(total, dtype=torch.float64, device="cuda")
+    for stage in (1, 2, 3, 4):
+        out_a = torch.full((total,), float("nan"), dtype=torch.float64, device="cuda")
+        out_b = torch.full((total,), float("nan"), dtype=torch.float64, device="cuda")
+        sacra.rk4_substep(ps, w.params, stage, un, uin, out_a, acc_a)
+        sacra.rk4_substep_part(ps, w.params, stage, sacra.PART_INTERIOR, faces, un, uin, out_b, acc_b)
+        mid = host(out_b).copy()
+        sacra.rk4_substep_part(ps, w.params, stage, sacra.PART_SHELL, faces, un, uin, out_b, acc_b)
+        a, b = host(out_a), host(out_b)
+        assert np.array_equal(np.isnan(a), np.isnan(b)) and np.array_equal(np.nan_to_num(a), np.nan_to_num(b)), stage
+        assert np.array_equal(host(acc_a), host(acc_b)), stage
+        if stage == 1:      # the interior part alone left exactly the shell cells untouched
+            p = ps[0]
+            v = w.active_view(mid, 0, 3)
+            i, j, k = np.arange(p.nx), np.arange(p.ny), np.arange(p.nz)
+            sx = (faces[0] & (i < 3)) | (faces[1] & (i >= p.nx - 3))
+            sy = (faces[2] & (j < 3)) | (faces[3] & (j >= p.ny - 3))
+            sz = (faces[4] & (k < 3)) | (faces[5] & (k >= p.nz - 3))
+            shell = sz.astype(bool)[:, None, None] | sy.astype(bool)[None, :, None] | sx.astype(bool)[None, None, :]
+            assert np.array_equal(np.isnan(v), shell)
+        nxt = out_a.clone()
+        sacra.fill_ghosts(ps, nxt)
+        uin = nxt
+
+
+def test_overlapped_distributed_step_equals_the_plain_step_bitwise():
+    w = _smooth(_w((33, 18, 20), seed=8))
+    p = w.patches[0]
+    topo = halo.CartTopology((1, 1, 1))
+    u, v = dev(w.state), dev(w.state)
+    n = u.numel()
+    wu, wv = torch.zeros(3 * n, dtype=torch.float64, device="cuda"), torch.zeros(3 * n, dtype=torch.float64, device="cuda")
+    bufs = {}
+    for _ in range(2):
+        halo.rk4_step_distributed(p, w.params, u, wu, topo, 0, buffers=bufs, overlap=True)
+        sacra.rk4_step([p], w.params, v, wv)
+        torch.cuda.synchronize()
+        assert np.array_equal(host(u), host(v)) and np.array_equal(host(wu[2 * n:]), host(wv[2 * n:]))
