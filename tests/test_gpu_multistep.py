@@ -42,8 +42,11 @@ def _gpu_norms(w, u, con, scratch, norms):
     return host(norms).copy()
 
 
-@pytest.mark.parametrize("idx,nsteps,quad_steps", [(0, 10, 3), (1, 10, 0)])
+@pytest.mark.parametrize("idx,nsteps,quad_steps", [(0, 10, 3), (1, 10, 0), (4, 3, 0)])
 def test_ten_consecutive_steps_beside_the_oracle(idx, nsteps, quad_steps):
+    """configs 0 and 1: ten steps. Config 4 (256^3, the timed workload): three consecutive steps on ALL points, the
+    most the two oracle trajectories allow within a minute of host time; no constraint norms there (the step-by-step
+    state comparison covers every field the norms are made of)."""
     w = wl.make(idx)
     ps, prm = w.patches, w.params
     n = w.state.size
@@ -77,6 +80,8 @@ def test_ten_consecutive_steps_beside_the_oracle(idx, nsteps, quad_steps):
                 if k <= quad_steps:
                     q = w.active_view(uQ, ip, f)
                     assert np.max(np.abs(a - q)) <= bound + np.max(np.abs(b - q)), (w.name, "quad", k, wl.FIELD_NAMES[f])
+        if idx == 4:
+            continue
         # constraint monitor on the evolved state: the CUDA norms of the CUDA state against the oracle's norms of its own
         ng = _gpu_norms(w, u, con, scratch, norms)
         no = orc.constraint_norms(ps, orc.constraints(ps, uA))
