@@ -485,65 +485,91 @@ __global__ void __launch_bounds__(128) k_restrict(const __grid_constant__ LevelP
            (long long)(L.org[1] + my + NG) * pp.pitch + (L.org[0] + mx + NG)] = az;
 }
 // prolongation of the child's ghost cells: 6 points per axis a quarter of a parent spacing off the parent cell that
-// holds the child cell (to the left for an even child cell, to the right for an odd one: mirrored weights)
-__device__ __forceinline__ void prolong_axis(int i, int org, int& j0, double (&w)[6]) {
-  const double we[6] = {63.0 / 8192.0, -495.0 / 8192.0, 2310.0 / 8192.0, 6930.0 / 8192.0, -693.0 / 8192.0, 77.0 / 8192.0};
-  const int m = i >> 1;                 // floor(i / 2), also for negative i
-  const bool odd = i & 1;
-  j0 = org + m + (odd ? -2 : -3);
-#pragma unroll
-  for (int k = 0; k < 6; ++k) w[k] = odd ? we[5 - k] : we[k];
-}
+// holds the child cell (to the left for an even child cell, to the right for an odd one: mirrored weights).
+// One thread per PARENT cell m = (mx, my, mz) of the child's storage range (m = -2 .. n/2 + 1 per axis) and field: the
+// up to eight child cells 2m + (0|1) it holds share the 7 x 7 x 7 parent values m - 3 .. m + 3 (an even child cell uses
+// the first six per axis, an odd one the last six with the mirrored weights), so the x sums of a parent row serve two
+// cells, the y sums four and a thread makes 343 loads for eight cells instead of 8 x 216. Every cell's sum is still
+// nested z(y(x)), terms in ascending order from 0.0: the same bits as the one-cell-per-thread form and as the oracle.
+// Only ghost cells are written; parent values that no ghost cell of the group needs are not loaded (they may lie
+// outside the parent's storage at the last group of an axis).
 __global__ void __launch_bounds__(128) k_prolong_ghosts(const __grid_constant__ LevelPair L, const double* __restrict__ u_parent,
                                                         double* __restrict__ u_child) {
   const DevPatch& pp = L.parent;
   const DevPatch& pc = L.child;
-  const int sx = pc.nx + 2 * NG, sy = pc.ny + 2 * NG;
-  // the ghost shell only: 6 whole z planes, then 6 whole rows of every active plane, then the 6 x-ghosts of every
-  // active row
-  const int nzs = 2 * NG * sx * sy, nys = 2 * NG * sx * pc.nz, nxs = 2 * NG * pc.ny * pc.nz;
+  const int gx = pc.nx / 2 + 4, gy = pc.ny / 2 + 4, gz = pc.nz / 2 + 4;     // parent cells that hold storage cells of the child
+  // the groups that hold ghost cells form a shell two parent cells thick: 4 whole z layers, then 4 rows of every other
+  // layer, then 4 cells of every other row (x fastest inside each part, so that a warp works on neighbouring groups)
+  const int nzs = 4 * gx * gy, nys = 4 * gx * (gz - 4), nxs = 4 * (gy - 4) * (gz - 4);
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= nzs + nys + nxs) return;
-  int I, J, Kk;
+  int m[3];
+  auto edge = [](int q, int g) { return q < 2 ? q - 2 : g - 6 + q; };   // q = 0..3 -> -2, -1, g - 4, g - 3
   if (t < nzs) {
-    I = t % sx; J = (t / sx) % sy;
-    const int q = t / (sx * sy);
-    Kk = q < NG ? q : pc.nz + q;
+    m[0] = t % gx - 2; m[1] = (t / gx) % gy - 2; m[2] = edge(t / (gx * gy), gz);
   } else if (t < nzs + nys) {
     t -= nzs;
-    I = t % sx;
-    const int q = (t / sx) % (2 * NG);
-    J = q < NG ? q : pc.ny + q;
-    Kk = t / (sx * 2 * NG) + NG;
+    m[0] = t % gx - 2; m[1] = edge((t / gx) % 4, gy); m[2] = t / (gx * 4);
   } else {
     t -= nzs + nys;
-    const int q = t % (2 * NG);
-    I = q < NG ? q : pc.nx + q;
-    J = (t / (2 * NG)) % pc.ny + NG;
-    Kk = t / (2 * NG * pc.ny) + NG;
+    m[0] = edge(t % 4, gx); m[1] = (t / 4) % (gy - 4); m[2] = t / (4 * (gy - 4));
   }
-  const int i = I - NG, j = J - NG, k = Kk - NG;
-  int x0, y0, z0;
-  double wx[6], wy[6], wz[6];
-  prolong_axis(i, L.org[0], x0, wx);
-  prolong_axis(j, L.org[1], y0, wy);
-  prolong_axis(k, L.org[2], z0, wz);
-  const double* fp = u_parent + pp.offset + (long long)blockIdx.y * pp.fstride + (long long)(z0 + NG) * pp.sz +
-                     (long long)(y0 + NG) * pp.pitch + (x0 + NG);
-  double az = 0.0;
+  const int nc[3] = {pc.nx, pc.ny, pc.nz};
+  // per axis and parity: is child cell i = 2m + parity inside the child's storage, and is it a ghost cell along that axis?
+  bool in[3][2], gh[3][2];
+  bool any_ghost_axis = false;
 #pragma unroll
-  for (int kz = 0; kz < 6; ++kz) {
-    double ay = 0.0;
+  for (int a = 0; a < 3; ++a)
 #pragma unroll
-    for (int ky = 0; ky < 6; ++ky) {
-      double ax = 0.0;
-#pragma unroll
-      for (int kx = 0; kx < 6; ++kx) ax = ax + wx[kx] * fp[(long long)kz * pp.sz + (long long)ky * pp.pitch + kx];
-      ay = ay + wy[ky] * ax;
+    for (int q = 0; q < 2; ++q) {
+      const int i = 2 * m[a] + q;
+      in[a][q] = i >= -NG && i < nc[a] + NG;
+      gh[a][q] = in[a][q] && (i < 0 || i >= nc[a]);
+      any_ghost_axis = any_ghost_axis || gh[a][q];
     }
-    az = az + wz[kz] * ay;
+  if (!any_ghost_axis) return;   // a group of active cells only
+  const double we[6] = {63.0 / 8192.0, -495.0 / 8192.0, 2310.0 / 8192.0, 6930.0 / 8192.0, -693.0 / 8192.0, 77.0 / 8192.0};
+  const double* fp = u_parent + pp.offset + (long long)blockIdx.y * pp.fstride + (long long)(L.org[2] + m[2] - 3 + NG) * pp.sz +
+                     (long long)(L.org[1] + m[1] - 3 + NG) * pp.pitch + (L.org[0] + m[0] - 3 + NG);
+  double az[2][2][2];            // [z parity][y parity][x parity]
+#pragma unroll
+  for (int c = 0; c < 8; ++c) az[c >> 2][(c >> 1) & 1][c & 1] = 0.0;
+#pragma unroll
+  for (int kz = 0; kz < 7; ++kz) {
+    // plane kz serves the even cell if kz < 6 and the odd one if kz > 0
+    if (!((kz < 6 && in[2][0]) || (kz > 0 && in[2][1]))) continue;
+    double ay[2][2];             // [y parity][x parity]
+    ay[0][0] = ay[0][1] = ay[1][0] = ay[1][1] = 0.0;
+#pragma unroll
+    for (int ky = 0; ky < 7; ++ky) {
+      if (!((ky < 6 && in[1][0]) || (ky > 0 && in[1][1]))) continue;
+      const double* row = fp + (long long)kz * pp.sz + (long long)ky * pp.pitch;
+      double v[7];
+#pragma unroll
+      for (int kx = 0; kx < 7; ++kx) v[kx] = ((kx < 6 && in[0][0]) || (kx > 0 && in[0][1])) ? row[kx] : 0.0;
+      double axe = 0.0, axo = 0.0;
+#pragma unroll
+      for (int kx = 0; kx < 6; ++kx) {
+        axe = axe + we[kx] * v[kx];            // even cell: nodes m-3 .. m+2
+        axo = axo + we[5 - kx] * v[kx + 1];    // odd cell:  nodes m-2 .. m+3, mirrored weights
+      }
+      if (ky < 6) { ay[0][0] = ay[0][0] + we[ky] * axe; ay[0][1] = ay[0][1] + we[ky] * axo; }
+      if (ky > 0) { ay[1][0] = ay[1][0] + we[6 - ky] * axe; ay[1][1] = ay[1][1] + we[6 - ky] * axo; }
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      if (kz < 6) az[0][c >> 1][c & 1] = az[0][c >> 1][c & 1] + we[kz] * ay[c >> 1][c & 1];
+      if (kz > 0) az[1][c >> 1][c & 1] = az[1][c >> 1][c & 1] + we[6 - kz] * ay[c >> 1][c & 1];
+    }
   }
-  u_child[pc.offset + (long long)blockIdx.y * pc.fstride + (long long)Kk * pc.sz + (long long)J * pc.pitch + I] = az;
+  double* fc = u_child + pc.offset + (long long)blockIdx.y * pc.fstride;
+#pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    const int qz = c >> 2, qy = (c >> 1) & 1, qx = c & 1;
+    if (!(in[0][qx] && in[1][qy] && in[2][qz])) continue;
+    if (!(gh[0][qx] || gh[1][qy] || gh[2][qz])) continue;       // an active cell
+    fc[(long long)(2 * m[2] + qz + NG) * pc.sz + (long long)(2 * m[1] + qy + NG) * pc.pitch + (2 * m[0] + qx + NG)] = az[qz][qy][qx];
+  }
 }
 
 // Halo exchange between the patches of a block decomposition ("pack, then non-blocking
@@ -1114,8 +1140,8 @@ int sacra_prolong_ghosts(const sacra_patch_t* parent, const sacra_patch_t* child
   if (!aligned16(u_parent) || !aligned16(u_child)) return SACRA_ERR_ALIGN;
   if (overlap(u_parent, state_extent(parent, 1), u_child, state_extent(child, 1))) return SACRA_ERR_BADARG;
   const LevelPair L = level_pair(parent, child, org);
-  const int sx = child->nx + 2 * NG, sy = child->ny + 2 * NG;
-  const int n = 2 * NG * (sx * sy + sx * child->nz + child->ny * child->nz);   // cells of the ghost shell
+  const int gx = child->nx / 2 + 4, gy = child->ny / 2 + 4, gz = child->nz / 2 + 4;
+  const int n = 4 * (gx * gy + gx * (gz - 4) + (gy - 4) * (gz - 4));   // parent cells that hold ghost cells of the child
   k_prolong_ghosts<<<dim3((n + 127) / 128, NF), 128, 0, static_cast<cudaStream_t>(cuda_stream)>>>(L, u_parent, u_child);
   return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
 }
@@ -1223,8 +1249,8 @@ int sacra_subcycle_step(const sacra_patch_t* parent, const sacra_patch_t* child,
   double* acc = work_child + 2 * child_doubles;
   const double cs[4] = {0.0, 0.5, 0.5, 1.0};
   const LevelPair L = level_pair(parent, child, org);
-  const int sx = child->nx + 2 * NG, sy = child->ny + 2 * NG;
-  const int nshell = 2 * NG * (sx * sy + sx * child->nz + child->ny * child->nz);
+  const int pgx = child->nx / 2 + 4, pgy = child->ny / 2 + 4, pgz = child->nz / 2 + 4;
+  const int nshell = 4 * (pgx * pgy + pgx * (pgz - 4) + (pgy - 4) * (pgz - 4));   // parent cells that hold ghost cells
   auto prolong = [&](const double* up, double* uc) {
     k_prolong_ghosts<<<dim3((nshell + 127) / 128, NF), 128, 0, st>>>(L, up, uc);
     return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
