@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- Z4c RHS + KO + RK4 throughput of libsacra on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference] [--all-configs]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference] [--headline-only]
 
 One "step" = one full RK4 step (5 halo fills + 4 fused RHS/KO/RK substages) of the whole workload through the
 C ABI call sacra_rk4_step. Default workload: BASELINE.json configs[4], one 256^3 periodic patch, 25 FP64 fields,
@@ -401,7 +401,7 @@ def run_ours(args):
                                "hbm_frac": 152.0 * npts / (con_ms * 1e-3) / 1e9 / hbm_gbs,
                                "norms_H_Mx_My_Mz": norms_host},
     }
-    if args.all_configs:
+    if args.all_configs and world == 1 and args.config == 4 and not args.n:
         out["configs"] = [measure_config(i, args, hbm_gbs, fp64_peak_tf) for i in range(4)]
     print(json.dumps(out))
 
@@ -466,8 +466,9 @@ def main():
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel (default: the committed ncu capture "
                          "profiles/r02_traffic.json if it was made for the current kernel sources)")
-    ap.add_argument("--all-configs", action="store_true",
-                    help="also time BASELINE.json configs 0-3 (one line: the headline stays config 4, plus `configs`)")
+    ap.add_argument("--all-configs", action="store_true", default=True,
+                    help="also time BASELINE.json configs 0-3 (default; the headline stays config 4, the line gains `configs`)")
+    ap.add_argument("--headline-only", dest="all_configs", action="store_false", help="skip configs 0-3")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
