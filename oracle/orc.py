@@ -257,3 +257,19 @@ def subcycle_step(parent, child, org, prm, bnd, u_parent, u_parent_prev, have_pr
     lib().orc_subcycle_step(C.byref(_patches([parent])[0]), C.byref(_patches([child])[0]), o, C.byref(pr),
                             C.byref(_boundaries([bnd])[0]), _p(u_parent), _p(u_parent_prev), int(bool(have_prev)),
                             _p(u_child), C.c_int64(u_parent.size), C.c_int64(u_child.size))
+
+
+def hierarchy_step(patches, orgs, prm, bnd0, states, prevs, nsteps):
+    """one step of level 0 of a hierarchy of nested levels (level l + 1 inside level l at parent index orgs[l + 1]; orgs[0]
+    unused), every finer level subcycled; in place on states / prevs (lists of arrays); nsteps: list of ints, updated"""
+    n = len(patches)
+    o = (C.c_int32 * (3 * n))(*[int(v) for org in orgs for v in org])
+    pr = _params(prm)
+    PP = C.POINTER(C.c_double)
+    us = (PP * n)(*[_p(a) for a in states])
+    ps_ = (PP * n)(*[_p(a) for a in prevs])
+    nd = (C.c_int64 * n)(*[a.size for a in states])
+    ns = (C.c_int64 * n)(*[int(v) for v in nsteps])
+    lib().orc_hierarchy_step(_patches(patches), o, n, C.byref(pr), C.byref(_boundaries([bnd0])[0]), us, ps_, nd, ns)
+    for i in range(n):
+        nsteps[i] = int(ns[i])

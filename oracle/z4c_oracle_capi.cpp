@@ -210,6 +210,21 @@ void orc_subcycle_step(const orc_patch* parent, const orc_patch* child, const in
                         u_parent_prev, have_prev != 0, u_child, n_parent, n_child);
 }
 
+// one step of the coarsest level of a hierarchy of nlevels nested levels (level l + 1 inside level l); arrays of nlevels
+// entries; nsteps is updated
+void orc_hierarchy_step(const orc_patch* patches, const int32_t* orgs /* 3 per level */, int nlevels, const orc_params* prm,
+                        const orc_boundary* bnd0, double* const* u, double* const* prev, const int64_t* ndoubles,
+                        int64_t* nsteps) {
+  std::vector<Level<double>> L(nlevels);
+  for (int l = 0; l < nlevels; ++l) {
+    L[l].p = to_patch(patches[l]);
+    for (int a = 0; a < 3; ++a) L[l].org[a] = orgs[3 * l + a];
+    L[l].u = u[l]; L[l].prev = prev[l]; L[l].n = ndoubles[l]; L[l].nsteps = nsteps[l];
+  }
+  hierarchy_advance<double>(L, 0, to_params<double>(*prm), to_boundary(*bnd0), 0);
+  for (int l = 0; l < nlevels; ++l) nsteps[l] = L[l].nsteps;
+}
+
 // ---- __float128 referee ------------------------------------------------------
 typedef __float128 Q;
 void orc_z4c_rhs_q(const orc_patch* ps, int np, const orc_params* prm, const double* u, double* rhs,

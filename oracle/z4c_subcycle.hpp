@@ -82,3 +82,72 @@ void subcycle_step(const Patch& pp, const Patch& pc, const int org[3], const Par
 }
 
 }  // namespace z4c_oracle
+
+// ---- hierarchy of nested levels ("fixed levels, each a single cubic patch"; level l + 1 is the child of
+// level l, half its spacing and time step). Recursive Berger-Oliger step, the pair step above applied at every level:
+//   step(0):   U_0 takes one RK4 step with its boundary modes.
+//   step(l>0): level l takes one RK4 step of dt_l; the ghosts of every substage input are prolonged from the parent's time
+//              levels (U^{n-1}, U^n, U^{n+1} of level l - 1; first order while the parent has no U^{n-1} yet) at
+//              theta = (m + c_s) / 2, m = 0, 1 the number of this step inside the parent's.
+//   after a step of level l: if it has a child, the child takes two steps (recursively), then the child's ghosts are
+//              prolonged from the new U_l, the child is restricted onto U_l and U_l's ghosts are refilled (level 0: its
+//              boundary modes; level l > 0: prolongation from its parent at the time just reached -- theta = (m + 1) / 2).
+// With two levels this is subcycle_step(), bit for bit.
+namespace z4c_oracle {
+
+template <class T> struct Level {
+  Patch p;
+  int org[3];          // position in the parent (unused for level 0)
+  T* u;                // state
+  T* prev;             // U^{n-1} of this level (valid when nsteps > 0)
+  long n;              // doubles per state
+  long nsteps;         // steps this level has taken
+  std::vector<T> old;  // U^n during a step
+};
+
+template <class T>
+void hierarchy_advance(std::vector<Level<T>>& L, int l, const Params<T>& P, const Boundary& b0, int m) {
+  Level<T>& me = L[l];
+  me.old.assign(me.u, me.u + me.n);
+  std::vector<T> wk(4 * me.n, T(0));
+  T* w0 = wk.data();
+  T* w1 = wk.data() + me.n;
+  T* acc = wk.data() + 2 * me.n;
+  T* kbuf = wk.data() + 3 * me.n;
+  auto parent_ghosts = [&](T theta, T* target) {      // ghosts of `target` from the parent's time levels at theta
+    Level<T>& pa = L[l - 1];
+    const int nlev = pa.nsteps > 0 ? 3 : 2;
+    const T* lev[3];
+    if (nlev == 3) { lev[0] = pa.prev; lev[1] = pa.old.data(); lev[2] = pa.u; }
+    else { lev[0] = pa.old.data(); lev[1] = pa.u; lev[2] = nullptr; }
+    T w[3];
+    time_weights<T>(nlev, theta, w);
+    std::vector<T> tmp(pa.n, T(0));
+    lincomb_patch<T>(pa.p, nlev, lev, w, tmp.data());
+    prolong_ghosts<T>(pa.p, me.p, me.org, tmp.data(), target);
+  };
+  if (l == 0) {
+    rk4_step_bc<T>(&me.p, &b0, 1, P, me.u, w0, w1, acc, kbuf);
+  } else {
+    const T cs[4] = {T(0), T(1) / T(2), T(1) / T(2), T(1)};
+    const T* in[4] = {me.u, w0, w1, w0};
+    T* out[4] = {w0, w1, w0, me.u};
+    for (int s = 0; s < 4; ++s) {
+      parent_ghosts((T(m) + cs[s]) / T(2), const_cast<T*>(in[s]));
+      rk4_substep<T>(me.p, P, s + 1, me.u, in[s], out[s], acc, kbuf);
+    }
+  }
+  if (l + 1 < (int)L.size()) {
+    hierarchy_advance<T>(L, l + 1, P, b0, 0);
+    hierarchy_advance<T>(L, l + 1, P, b0, 1);
+    Level<T>& ch = L[l + 1];
+    prolong_ghosts<T>(me.p, ch.p, ch.org, me.u, ch.u);
+    restrict_patch<T>(me.p, ch.p, ch.org, me.u, ch.u);
+  }
+  if (l == 0) fill_ghosts_faces<T>(me.p, b0.face, me.u);
+  else parent_ghosts((T(m) + T(1)) / T(2), me.u);
+  for (long i = 0; i < me.n; ++i) me.prev[i] = me.old[i];
+  me.nsteps += 1;
+}
+
+}  // namespace z4c_oracle
