@@ -223,6 +223,27 @@ int sacra_subcycle_step(const sacra_patch_t* parent, const sacra_patch_t* child,
                         double* u_parent_prev, int have_prev, double* u_child, double* work_parent,
                         int64_t parent_doubles, double* work_child, int64_t child_doubles, void* cuda_stream);
 
+/* A hierarchy of nested levels ("fixed levels, each a single cubic patch"): level l + 1 is the child of
+ * level l (half its spacing, half its time step, nested at parent index org). One call advances level 0 by one step and
+ * every finer level by its two, four, ... steps, recursively: the pair step above applied at every level -- a level takes
+ * its RK4 step (level 0 with its boundary modes; level l > 0 with the ghosts of every substage input prolonged from its
+ * parent's time levels U^n-1, U^n, U^n+1 at the substage time, first order while the parent has no U^n-1 yet), then its
+ * child takes two steps, the child is restricted onto it and its own ghosts are refilled (level 0: boundary modes;
+ * l > 0: from the parent at the time just reached). With two levels this is sacra_subcycle_step, bit for bit.
+ * levels: HOST array of nlevels entries (<= 16), updated (nsteps). All pointers inside are as described per field. */
+typedef struct {
+  const sacra_patch_t* patch; /* HOST: the level's patch                                                            */
+  int32_t org[3];             /* position in the parent, as for sacra_prolong_ghosts (level 0: ignored)             */
+  int32_t pad_;               /* set to 0                                                                           */
+  double* u;                  /* DEVICE: the level's state (ghosts valid on entry and on return)                    */
+  double* u_prev;             /* DEVICE: U^n-1 of the level; written by every step, read when nsteps > 0            */
+  double* work;               /* DEVICE: 5 x state_doubles                                                          */
+  int64_t state_doubles;
+  int64_t nsteps;             /* steps the level has taken so far (0 at the start of a run); updated by the call    */
+} sacra_level_t;
+int sacra_hierarchy_step(sacra_level_t* levels, int nlevels, const sacra_params_t* prm, const sacra_boundary_t* bnd0,
+                         void* cuda_stream);
+
 /* Halo exchange between the patches of a block decomposition over several GPUs (the
  * 3 ghost layers of every field at every face are packed into a buffer and exchanged with the neighbouring rank before
  * each RK substage). ONE patch per call. axis 0, 1, 2 = x, y, z; side 0 = low face, 1 = high face.

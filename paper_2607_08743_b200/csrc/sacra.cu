@@ -1284,6 +1284,111 @@ int sacra_subcycle_step(const sacra_patch_t* parent, const sacra_patch_t* child,
   return SACRA_OK;
 }
 
+// Recursive Berger-Oliger step (sacra.h: sacra_hierarchy_step). Level l's buffers: old = work, tmp = work + n (its data
+// interpolated in time for its child), then w0, w1, acc of its RK4 step.
+namespace {
+struct HierCtx {
+  sacra_level_t* L;
+  int nlevels;
+  const sacra_params_t* prm;
+  const sacra_boundary_t* bnd0;
+  cudaStream_t st;
+};
+// ghosts of `target` (a state of level l) from the time levels of level l - 1 at theta
+int hier_parent_ghosts(const HierCtx& c, int l, double theta, double* target) {
+  sacra_level_t& pa = c.L[l - 1];
+  sacra_level_t& me = c.L[l];
+  const int nlev = pa.nsteps > 0 ? 3 : 2;
+  double* old = pa.work;
+  double* tmp = pa.work + pa.state_doubles;
+  const double* lev[3] = {nlev == 3 ? pa.u_prev : old, nlev == 3 ? old : pa.u, nlev == 3 ? pa.u : nullptr};
+  double w[3];
+  sacra_time_weights(nlev, theta, w);
+  int blo[3], bhi[3];
+  const int ncs[3] = {me.patch->nx, me.patch->ny, me.patch->nz};
+  for (int a = 0; a < 3; ++a) {
+    blo[a] = me.org[a] - 5 + NG;
+    bhi[a] = me.org[a] + ncs[a] / 2 + 3 + NG + 1;
+  }
+  if (int e = launch_lincomb(pa.patch, nlev, lev[0], lev[1], lev[2], w, tmp, c.st, blo, bhi)) return e;
+  const LevelPair P = level_pair(pa.patch, me.patch, me.org);
+  const int gx = ncs[0] / 2 + 4, gy = ncs[1] / 2 + 4, gz = ncs[2] / 2 + 4;
+  const int n = 4 * (gx * gy + gx * (gz - 4) + (gy - 4) * (gz - 4));
+  k_prolong_ghosts<<<dim3((n + 127) / 128, NF), 128, 0, c.st>>>(P, tmp, target);
+  return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
+}
+int hier_advance(const HierCtx& c, int l, int m) {
+  sacra_level_t& me = c.L[l];
+  const int64_t n = me.state_doubles;
+  double* old = me.work;
+  double* w0 = me.work + 2 * n;
+  double* w1 = me.work + 3 * n;
+  double* acc = me.work + 4 * n;
+  int e;
+  if (cudaMemcpyAsync(old, me.u, (size_t)n * 8, cudaMemcpyDeviceToDevice, c.st) != cudaSuccess) return SACRA_ERR_CUDA;
+  if (l == 0) {
+    if ((e = sacra_rk4_step_bc(me.patch, 1, c.prm, c.bnd0, me.u, w0, n, c.st))) return e;
+  } else {
+    const double cs[4] = {0.0, 0.5, 0.5, 1.0};
+    const double* in[4] = {me.u, w0, w1, w0};
+    double* out[4] = {w0, w1, w0, me.u};
+    for (int s = 0; s < 4; ++s) {
+      if ((e = hier_parent_ghosts(c, l, ((double)m + cs[s]) / 2.0, const_cast<double*>(in[s])))) return e;
+      if ((e = launch_z4c(me.patch, 1, c.prm, s + 1, in[s], nullptr, me.u, out[s], acc, c.st))) return e;
+    }
+  }
+  if (l + 1 < c.nlevels) {
+    if ((e = hier_advance(c, l + 1, 0))) return e;
+    if ((e = hier_advance(c, l + 1, 1))) return e;
+    sacra_level_t& ch = c.L[l + 1];
+    if ((e = sacra_prolong_ghosts(me.patch, ch.patch, ch.org, me.u, ch.u, c.st))) return e;
+    if ((e = sacra_restrict(me.patch, ch.patch, ch.org, me.u, ch.u, c.st))) return e;
+  }
+  if (l == 0) {
+    if ((e = launch_fill(me.patch, 1, me.u, c.st, nullptr, c.bnd0))) return e;
+  } else if ((e = hier_parent_ghosts(c, l, ((double)m + 1.0) / 2.0, me.u))) {
+    return e;
+  }
+  if (cudaMemcpyAsync(me.u_prev, old, (size_t)n * 8, cudaMemcpyDeviceToDevice, c.st) != cudaSuccess) return SACRA_ERR_CUDA;
+  me.nsteps += 1;
+  return SACRA_OK;
+}
+}  // namespace
+
+int sacra_hierarchy_step(sacra_level_t* levels, int nlevels, const sacra_params_t* prm, const sacra_boundary_t* bnd0,
+                         void* cuda_stream) {
+  if (!levels || !prm || !bnd0) return SACRA_ERR_NULL;
+  if (nlevels < 1 || nlevels > 16) return SACRA_ERR_BADARG;
+  if (int e = check_boundaries(bnd0, 1)) return e;
+  for (int l = 0; l < nlevels; ++l) {
+    const sacra_level_t& a = levels[l];
+    if (!a.patch || !a.u || !a.u_prev || !a.work) return SACRA_ERR_NULL;
+    if (int e = check_patches(a.patch, 1)) return e;
+    if (a.state_doubles < state_extent(a.patch, 1) || (a.state_doubles & 1) || a.nsteps < 0) return SACRA_ERR_BADARG;
+    if (!aligned16(a.u) || !aligned16(a.u_prev) || !aligned16(a.work)) return SACRA_ERR_ALIGN;
+    if (overlap(a.u, a.state_doubles, a.u_prev, a.state_doubles) || overlap(a.u, a.state_doubles, a.work, 5 * a.state_doubles) ||
+        overlap(a.u_prev, a.state_doubles, a.work, 5 * a.state_doubles))
+      return SACRA_ERR_BADARG;
+    if (l > 0) {
+      const sacra_level_t& pa = levels[l - 1];
+      if (int e = check_levels(pa.patch, a.patch, a.org, true)) return e;
+      if (std::fabs(2.0 * a.patch->dt - pa.patch->dt) > 1e-12 * std::fabs(pa.patch->dt)) return SACRA_ERR_BADARG;
+      for (int k = 0; k < l; ++k) {      // buffers of different levels are disjoint
+        const sacra_level_t& b = levels[k];
+        const double* A[3] = {a.u, a.u_prev, a.work};
+        const double* Bq[3] = {b.u, b.u_prev, b.work};
+        const long long na[3] = {a.state_doubles, a.state_doubles, 5 * a.state_doubles};
+        const long long nb[3] = {b.state_doubles, b.state_doubles, 5 * b.state_doubles};
+        for (int i = 0; i < 3; ++i)
+          for (int j = 0; j < 3; ++j)
+            if (overlap(A[i], na[i], Bq[j], nb[j])) return SACRA_ERR_BADARG;
+      }
+    }
+  }
+  HierCtx c{levels, nlevels, prm, bnd0, static_cast<cudaStream_t>(cuda_stream)};
+  return hier_advance(c, 0, 0);
+}
+
 const char* sacra_strerror(int code) {
   switch (code) {
     case SACRA_OK: return "ok";

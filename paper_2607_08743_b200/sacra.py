@@ -24,7 +24,8 @@ EXPORTS = ("sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4
            "sacra_fill_ghosts_bc", "sacra_restrict", "sacra_prolong_ghosts",
            "sacra_fill_ghosts_faces", "sacra_sommerfeld_rhs", "sacra_rk4_substep_bc", "sacra_rk4_step_bc",
            "sacra_time_weights", "sacra_lincomb", "sacra_subcycle_step",
-           "sacra_face_doubles", "sacra_pack_face", "sacra_unpack_face", "sacra_rk4_substep_part")
+           "sacra_face_doubles", "sacra_pack_face", "sacra_unpack_face", "sacra_rk4_substep_part",
+           "sacra_hierarchy_step")
 
 
 class SacraPatch(C.Structure):
@@ -44,6 +45,12 @@ class SacraParams(C.Structure):
 class SacraBoundary(C.Structure):
     """sacra_boundary_t"""
     _fields_ = [("origin", C.c_double * 3), ("face", C.c_int32 * 6)]
+
+
+class SacraLevel(C.Structure):
+    """sacra_level_t"""
+    _fields_ = [("patch", C.POINTER(SacraPatch)), ("org", C.c_int32 * 3), ("pad_", C.c_int32), ("u", C.c_void_p),
+                ("u_prev", C.c_void_p), ("work", C.c_void_p), ("state_doubles", C.c_int64), ("nsteps", C.c_int64)]
 
 
 class SacraError(RuntimeError):
@@ -80,7 +87,8 @@ def _load():
     lib.sacra_pack_face.argtypes = [vp, dp, i32, i32, dp, vp]
     lib.sacra_unpack_face.argtypes = [vp, dp, i32, i32, dp, vp]
     lib.sacra_rk4_substep_part.argtypes = [vp, i32, vp, i32, i32, vp, dp, dp, dp, dp, vp]
-    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:19] + EXPORTS[20:23]:
+    lib.sacra_hierarchy_step.argtypes = [vp, i32, vp, vp, vp]
+    for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:19] + EXPORTS[20:24]:
         getattr(lib, n).restype = C.c_int
     lib.sacra_strerror.argtypes = [C.c_int]
     lib.sacra_strerror.restype = C.c_char_p
@@ -307,3 +315,21 @@ def rk4_substep_part(patches, params, stage, part, exchange_faces, u_n, u_in, u_
     xf = (C.c_int32 * 6)(*[int(v) for v in exchange_faces]) if exchange_faces is not None else None
     _check(lib.sacra_rk4_substep_part(ps, len(ps) if ps is not None else 0, _ref(pr), int(stage), int(part), xf,
                                       _ptr(u_n), _ptr(u_in), _ptr(u_out), _ptr(acc), _stream(stream)))
+
+
+def hierarchy_step(patches, orgs, params, bnd0, states, prevs, works, nsteps, stream=None):
+    """one step of level 0 of a hierarchy of nested levels, finer levels subcycled (sacra_hierarchy_step). patches, orgs,
+    states, prevs, works (5 states each): one entry per level; nsteps: list of ints, updated in place"""
+    n = len(patches)
+    keep = [make_patches([p]) for p in patches]
+    lv = (SacraLevel * n)()
+    for l in range(n):
+        lv[l].patch = C.cast(keep[l], C.POINTER(SacraPatch))
+        for a in range(3):
+            lv[l].org[a] = int(orgs[l][a])
+        lv[l].u, lv[l].u_prev, lv[l].work = _ptr(states[l]), _ptr(prevs[l]), _ptr(works[l])
+        lv[l].state_doubles, lv[l].nsteps = int(states[l].numel()), int(nsteps[l])
+    pr = make_params(params) if params is not None else None
+    _check(lib.sacra_hierarchy_step(lv, n, _ref(pr), make_boundaries([bnd0]), _stream(stream)))
+    for l in range(n):
+        nsteps[l] = int(lv[l].nsteps)

@@ -213,3 +213,36 @@ def test_partial_substep_and_face_buffer_argument_checks():
     assert _code(sacra.pack_face, ps[0], FAKE, 0, 2, far(1)) == sacra.ERR_BADARG
     assert _code(sacra.unpack_face, ps[0], FAKE, 0, 0, FAKE + 64) == sacra.ERR_BADARG                             # buffer inside the state
     assert _code(sacra.unpack_face, ps[0], None, 0, 0, far(1)) == sacra.ERR_NULL
+
+
+def test_hierarchy_argument_checks():
+    assert C.sizeof(sacra.SacraLevel) == 64
+    pp, tp = wl.make_layout([(16, 16, 16)], [0.2], [0.05], [(0, 0, 0)])
+    pc, tc = wl.make_layout([(8, 8, 8)], [0.1], [0.025], [(0, 0, 0)])
+    bnd = ((0.0, 0.0, 0.0), [0] * 6)
+    class T:                       # stand-in for a tensor: pointer and size
+        def __init__(self, ptr, n): self.ptr, self.n = ptr, n
+        def numel(self): return self.n
+    def lv(base, n):
+        step = 8 * (n + 64)
+        return base, base + step, base + 2 * step, base + 8 * step
+    a0, a1, a2, nxt = lv(FAKE, tp)
+    b0, b1, b2, _ = lv(nxt, tc)
+    def call(patches, orgs, bufs, sizes):
+        n = len(patches)
+        keep = [sacra.make_patches([p]) for p in patches]
+        arr = (sacra.SacraLevel * n)()
+        for l in range(n):
+            arr[l].patch = C.cast(keep[l], C.POINTER(sacra.SacraPatch))
+            for a in range(3):
+                arr[l].org[a] = orgs[l][a]
+            arr[l].u, arr[l].u_prev, arr[l].work = bufs[l]
+            arr[l].state_doubles, arr[l].nsteps = sizes[l], 0
+        return sacra.lib.sacra_hierarchy_step(arr, n, C.byref(sacra.make_params(PRM)), sacra.make_boundaries([bnd]), 0)
+    ok = [(0, 0, 0), (4, 4, 4)]
+    assert call([pp[0], pc[0]], ok, [(a0, a1, None), (b0, b1, b2)], [tp, tc]) == sacra.ERR_NULL
+    assert call([pp[0], pc[0]], [(0, 0, 0), (1, 4, 4)], [(a0, a1, a2), (b0, b1, b2)], [tp, tc]) == sacra.ERR_BADARG   # geometry
+    assert call([pp[0], pc[0]], ok, [(a0, a1, a2), (a0 + 64, b1, b2)], [tp, tc]) == sacra.ERR_BADARG                  # levels overlap
+    assert call([pp[0], pc[0]], ok, [(a0, a0 + 64, a2), (b0, b1, b2)], [tp, tc]) == sacra.ERR_BADARG                  # u / u_prev overlap
+    assert call([pp[0], pc[0]], ok, [(a0, a1, a2), (b0, b1, b2)], [tp, 100]) == sacra.ERR_BADARG                      # state too small
+    assert sacra.lib.sacra_hierarchy_step(None, 2, C.byref(sacra.make_params(PRM)), sacra.make_boundaries([bnd]), 0) == sacra.ERR_NULL
