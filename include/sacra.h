@@ -44,7 +44,9 @@ typedef enum {
   SACRA_ERR_UNSUPPORTED = -3, /* ng != 3                                                           */
   SACRA_ERR_ALIGN = -4,       /* pointer not 16-byte aligned, or pitch_x/field_stride/patch_offset
                                  breaks the 16-byte row alignment rule below                       */
-  SACRA_ERR_CUDA = -5         /* a CUDA launch failed (cudaGetLastError)                           */
+  SACRA_ERR_CUDA = -5,        /* a CUDA launch failed (cudaGetLastError)                           */
+  SACRA_ERR_TOOLARGE = -6     /* the problem exceeds a fixed capacity of the library
+                                 (sacra_constraint_norms_static: SACRA_NORMS_STATIC_MAX_PLANES)    */
 } sacra_status;
 
 /* One uniform, cell-centred patch (every box of the hierarchy is such a patch). */
@@ -179,6 +181,34 @@ int sacra_constraints(const sacra_patch_t* p, int npatch, const double* u, doubl
 int sacra_constraint_norms(const sacra_patch_t* p, int npatch, const double* con, double* scratch, double* norms,
                            void* cuda_stream);
 int64_t sacra_constraint_scratch_doubles(const sacra_patch_t* p, int npatch);
+
+/* The same norms for callers that have no device memory left to give and may not ask the CUDA runtime for more.
+ * Who that is: an evolution code sizes its state buffers to fill the GPU at start-up and hands everything to its own
+ * arena; the monitor is then called from inside the time loop every step, where a cudaMalloc is not
+ * an option - it synchronises the whole device, which stalls the streams that overlap the halo exchange with the
+ * substage kernels - and where there may simply be nothing left to allocate. sacra_constraint_norms asks such a
+ * caller for a scratch buffer; this call does not.
+ *
+ * Same arguments as sacra_constraint_norms without `scratch`, same kernels, same reduction order, hence the same bits
+ * in `norms`. The per-plane partial sums go to an array that lives inside the library image: 4 x
+ * SACRA_NORMS_STATIC_MAX_PLANES doubles = 128 KiB of device memory, held by every GPU that loads libsacra from
+ * the moment it loads it until the process exits, whether this call is used or not.
+ *
+ *   - Limit: the active z-planes of all patches together (sum of nz) must not exceed
+ *     SACRA_NORMS_STATIC_MAX_PLANES; otherwise SACRA_ERR_TOOLARGE is returned and nothing is launched. (256^3 has
+ *     256 planes, the 8 x 64^3 batch 512.) Larger batches: sacra_constraint_norms with the caller's buffer.
+ *   - The call itself calls no cudaMalloc / cudaFree and no library routine that allocates.
+ *   - First call on each device: with that device current, the library looks the array's device address up
+ *     (cudaGetSymbolAddress, return code checked -> SACRA_ERR_CUDA) and keeps it; later calls on that device reuse
+ *     it. Make this first call during set-up, outside any stream capture.
+ *   - All calls on one device share the one array, and it keeps what the last call left in it. Nothing in it has to
+ *     start at zero: each call overwrites every entry it later reads, so stale contents are harmless and nothing is
+ *     cleared. Two calls whose kernels can run at the same time on the same device (different streams, no
+ *     dependency between them) race on the array and give garbage in both `norms`; order them on one stream or with
+ *     an event. */
+#define SACRA_NORMS_STATIC_MAX_PLANES 4096
+int sacra_constraint_norms_static(const sacra_patch_t* p, int npatch, const double* con, double* norms,
+                                  void* cuda_stream);
 
 /* Spatial inter-level operators of the box-in-box hierarchy, 2:1 refinement on
  * cell-centred staggered grids. `parent` and `child` are ONE patch each (HOST pointers; the child has half the

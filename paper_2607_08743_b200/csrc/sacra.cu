@@ -891,6 +891,36 @@ static int launch_z4c(const sacra_patch_t* p, int npatch, const sacra_params_t* 
 
 using namespace sacra;
 
+// ---------------------------------------------------------------------------------------------------
+// Scratch of sacra_constraint_norms_static (sacra.h): the per-plane partial sums of k_con_partial for callers that
+// cannot provide a device buffer. It sits in the library image, so every GPU that loads libsacra carries these
+// 128 KiB until the process ends. One array per device, shared by all calls on that device.
+// In HOST code the name `con_part_static` is only a handle for the runtime, not a device address: a kernel handed
+// `con_part_static` itself would write to the wrong place. static_norm_scratch() asks the runtime for the real
+// address, once per device and with that device current, and remembers it.
+// ---------------------------------------------------------------------------------------------------
+static __device__ __align__(256) double con_part_static[4 * SACRA_NORMS_STATIC_MAX_PLANES];
+
+static const int STATIC_MAXDEV = 64;
+static std::mutex static_scratch_mutex;
+static double* static_scratch_addr[STATIC_MAXDEV];   // zero-initialised: not looked up yet
+
+// device address of con_part_static on the current device; nullptr if the runtime refuses
+static double* static_norm_scratch() {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= STATIC_MAXDEV) return nullptr;
+  std::lock_guard<std::mutex> lock(static_scratch_mutex);
+  if (!static_scratch_addr[dev]) {
+    double* ptr = nullptr;
+    if (cudaGetSymbolAddress((void**)&ptr, con_part_static) != cudaSuccess) {
+      (void)cudaGetLastError();   // leave no sticky error behind for the caller's next launch check
+      return nullptr;
+    }
+    static_scratch_addr[dev] = ptr;
+  }
+  return static_scratch_addr[dev];
+}
+
 extern "C" {
 
 int sacra_fill_ghosts(const sacra_patch_t* p, int npatch, double* u, void* cuda_stream) {
@@ -1095,6 +1125,22 @@ int sacra_constraint_norms(const sacra_patch_t* p, int npatch, const double* con
   }
   k_con_final<<<1, 4, 0, st>>>(scratch, planes, vol, norms);
   return cudaGetLastError() == cudaSuccess ? SACRA_OK : SACRA_ERR_CUDA;
+}
+
+// sacra_constraint_norms for callers that cannot allocate (sacra.h has the contract): the capacity check comes
+// first, so a batch that is too large launches nothing; then the partial sums go to the library's own array through
+// the unchanged path above. No allocation happens here or below. The array's old contents do not matter:
+// k_con_partial writes entries 0 .. 4*planes-1 and k_con_final reads exactly those.
+int sacra_constraint_norms_static(const sacra_patch_t* p, int npatch, const double* con, double* norms,
+                                  void* cuda_stream) {
+  if (!p || !con || !norms) return SACRA_ERR_NULL;
+  if (int e = check_patches(p, npatch)) return e;
+  int64_t planes = 0;
+  for (int q = 0; q < npatch; ++q) planes += p[q].nz;
+  if (planes > SACRA_NORMS_STATIC_MAX_PLANES) return SACRA_ERR_TOOLARGE;
+  double* part = static_norm_scratch();   // first call on this device: cudaGetSymbolAddress
+  if (!part) return SACRA_ERR_CUDA;
+  return sacra_constraint_norms(p, npatch, con, part, norms, cuda_stream);
 }
 
 // f-3: geometry checks shared by the two inter-level calls
@@ -1397,6 +1443,7 @@ const char* sacra_strerror(int code) {
     case SACRA_ERR_UNSUPPORTED: return "unsupported ghost width (ng must be 3)";
     case SACRA_ERR_ALIGN: return "pointer or layout breaks the 16-byte alignment rule";
     case SACRA_ERR_CUDA: return "CUDA launch failed";
+    case SACRA_ERR_TOOLARGE: return "problem exceeds a fixed capacity of the library (see sacra.h)";
     default: return "unknown sacra status";
   }
 }

@@ -16,7 +16,8 @@ from . import build as _build
 
 NF = 25
 NG = 3
-OK, ERR_NULL, ERR_BADARG, ERR_UNSUPPORTED, ERR_ALIGN, ERR_CUDA = 0, -1, -2, -3, -4, -5
+OK, ERR_NULL, ERR_BADARG, ERR_UNSUPPORTED, ERR_ALIGN, ERR_CUDA, ERR_TOOLARGE = 0, -1, -2, -3, -4, -5, -6
+NORMS_STATIC_MAX_PLANES = 4096
 FLAG_SKIP_INCREMENT = 1
 EXPORTS = ("sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4_step",
            "sacra_strerror", "sacra_version",
@@ -25,7 +26,7 @@ EXPORTS = ("sacra_fill_ghosts", "sacra_z4c_rhs", "sacra_rk4_substep", "sacra_rk4
            "sacra_fill_ghosts_faces", "sacra_sommerfeld_rhs", "sacra_rk4_substep_bc", "sacra_rk4_step_bc",
            "sacra_time_weights", "sacra_lincomb", "sacra_subcycle_step",
            "sacra_face_doubles", "sacra_pack_face", "sacra_unpack_face", "sacra_rk4_substep_part",
-           "sacra_hierarchy_step")
+           "sacra_hierarchy_step", "sacra_constraint_norms_static")
 
 
 class SacraPatch(C.Structure):
@@ -88,6 +89,8 @@ def _load():
     lib.sacra_unpack_face.argtypes = [vp, dp, i32, i32, dp, vp]
     lib.sacra_rk4_substep_part.argtypes = [vp, i32, vp, i32, i32, vp, dp, dp, dp, dp, vp]
     lib.sacra_hierarchy_step.argtypes = [vp, i32, vp, vp, vp]
+    lib.sacra_constraint_norms_static.argtypes = [vp, i32, dp, dp, vp]
+    lib.sacra_constraint_norms_static.restype = C.c_int
     for n in EXPORTS[:4] + EXPORTS[6:8] + EXPORTS[9:19] + EXPORTS[20:24]:
         getattr(lib, n).restype = C.c_int
     lib.sacra_strerror.argtypes = [C.c_int]
@@ -198,6 +201,17 @@ def constraint_norms(patches, con, scratch, norms, stream=None):
     ps = make_patches(patches) if patches is not None else None
     _check(lib.sacra_constraint_norms(ps, len(ps) if ps is not None else 0, _ptr(con), _ptr(scratch), _ptr(norms),
                                       _stream(stream)))
+
+
+def constraint_norms_static(patches, con, norms, stream=None):
+    """constraint_norms without the scratch argument, for callers that cannot allocate device memory (an arena owns
+    it all, or a cudaMalloc inside the time loop would stall the device). The partial sums go to a fixed 128 KiB
+    array inside libsacra that all calls on a device share: at most NORMS_STATIC_MAX_PLANES active z-planes over all
+    patches (SacraError with ERR_TOOLARGE beyond that), and calls that overlap on the GPU race. Same bits in `norms` as
+    constraint_norms. The first call on a device looks the array's address up; make it before any stream capture."""
+    ps = make_patches(patches) if patches is not None else None
+    _check(lib.sacra_constraint_norms_static(ps, len(ps) if ps is not None else 0, _ptr(con), _ptr(norms),
+                                             _stream(stream)))
 
 
 BC_PERIODIC, BC_MIRROR, BC_SOMMERFELD, BC_NONE = 0, 1, 2, 3

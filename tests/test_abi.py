@@ -36,8 +36,20 @@ def test_struct_layout_matches_header():
 
 
 def test_strerror_covers_every_code():
-    seen = {sacra.strerror(c) for c in range(0, -6, -1)}
-    assert len(seen) == 6 and sacra.strerror(-99) not in seen
+    seen = {sacra.strerror(c) for c in range(0, -7, -1)}
+    assert len(seen) == 7 and sacra.strerror(-99) not in seen
+
+
+def test_static_norms_capacity_is_checked_before_the_device_is_touched():
+    """sacra_constraint_norms_static (for callers that cannot allocate): more active z-planes than its fixed array
+    holds is SACRA_ERR_TOOLARGE, decided on the host, so it is testable without a GPU"""
+    hdr = open(os.path.join(ROOT, "include", "sacra.h")).read()
+    assert int(re.search(r"#define SACRA_NORMS_STATIC_MAX_PLANES (\d+)", hdr).group(1)) == sacra.NORMS_STATIC_MAX_PLANES
+    ps, _ = wl.make_layout([(6, 6, sacra.NORMS_STATIC_MAX_PLANES + 1)], [0.1], [0.025], [(0, 0, 0)])
+    assert _code(sacra.constraint_norms_static, ps, FAKE, FAKE) == sacra.ERR_TOOLARGE
+    ps, _ = wl.make_layout([(6, 6, 2048)] * 3, [0.1] * 3, [0.025] * 3, [(0, 0, 0)] * 3)
+    assert _code(sacra.constraint_norms_static, ps, FAKE, FAKE) == sacra.ERR_TOOLARGE
+    assert _code(sacra.constraint_norms_static, ps, None, FAKE) == sacra.ERR_NULL
 
 
 def _patch(**kw):
