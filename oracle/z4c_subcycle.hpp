@@ -89,7 +89,8 @@ void subcycle_step(const Patch& pp, const Patch& pc, const int org[3], const Par
 //   step(l>0): level l takes one RK4 step of dt_l; the ghosts of every substage input are prolonged from the parent's time
 //              levels (U^{n-1}, U^n, U^{n+1} of level l - 1; first order while the parent has no U^{n-1} yet) at
 //              theta = (m + c_s) / 2, m = 0, 1 the number of this step inside the parent's.
-//   after a step of level l: if it has a child, the child takes two steps (recursively), then the child's ghosts are
+//   after a step of level l: if it has a child, level l > 0 first refills its own ghosts at the time just reached (the
+//              child's prolongation box may read them), the child takes two steps (recursively), then the child's ghosts are
 //              prolonged from the new U_l, the child is restricted onto U_l and U_l's ghosts are refilled (level 0: its
 //              boundary modes; level l > 0: prolongation from its parent at the time just reached -- theta = (m + 1) / 2).
 // With two levels this is subcycle_step(), bit for bit.
@@ -138,6 +139,12 @@ void hierarchy_advance(std::vector<Level<T>>& L, int l, const Params<T>& P, cons
     }
   }
   if (l + 1 < (int)L.size()) {
+    // An intermediate level refreshes its own ghosts at the time just reached BEFORE its child advances: stage 4
+    // wrote active cells only, and the child's time-interpolated prolongation box (parent cells org - 4 ..
+    // org + n/2 + 3) reaches into these ghosts when the child sits within 4 cells of this level's edge. (Level 0's
+    // rk4_step_bc ends with its own fill.) PAPER.md:109: the child's buffer data come from the parent AT the
+    // substage's time, which needs every parent cell the stencil reads to be at U^{n+1}.
+    if (l > 0) parent_ghosts((T(m) + T(1)) / T(2), me.u);
     hierarchy_advance<T>(L, l + 1, P, b0, 0);
     hierarchy_advance<T>(L, l + 1, P, b0, 1);
     Level<T>& ch = L[l + 1];
