@@ -101,7 +101,8 @@ int sacra_fill_ghosts_bc(const sacra_patch_t* p, int npatch, const int32_t* axis
  * axis or on neither); SACRA_BC_SOMMERFELD: outer boundary with the outgoing-wave condition Eq. 13;
  * SACRA_BC_NONE: the ghost cells behind the face belong to somebody else (e.g. sacra_prolong_ghosts) and are left alone.
  * origin: coordinates of the centre of active cell (0,0,0); active cell (i,j,k) sits at origin + (i,j,k) dx (Eq. 13
- * needs x^i / r; the origin of the coordinates must not be a cell of a boundary shell).
+ * needs x^i / r; the origin of the coordinates must not be a cell of a Sommerfeld boundary shell: every call that
+ * evaluates Eq. 13 returns SACRA_ERR_BADARG, before launching anything, if such a cell has r = 0).
  * Reading of Eq. 13 (the paper gives no discretisation): on the BOUNDARY SHELL -- the active cells
  * within 3 cells of a SOMMERFELD face -- the right-hand side of all 25 fields is
  *     d_t Q = -( x^i d_i Q + Q ) / r,   Q = field - flat value (1 for W, gt_xx, gt_yy, gt_zz, alpha; 0 otherwise),

@@ -178,9 +178,24 @@ __global__ void __launch_bounds__(256) k_sommerfeld(const __grid_constant__ Patc
   const bool flat1 = f == F_W || f == F_G || f == F_G + 3 || f == F_G + 5 || f == F_ALP;
   const long long fo = p.offset + (long long)f * p.fstride;
   const double z = G.origin[ip][2] + (double)k * h;
-  for (int q = threadIdx.x; q < p.nx * p.ny; q += blockDim.x) {
-    const int i = q % p.nx, j = q / p.nx;
-    if (!in_shell(p.shell, p, i, j, k)) continue;
+  // Only the shell cells of plane k are visited (at 256^3 the shell is 7 % of the cells): a plane inside a z-shell is
+  // shell as a whole; elsewhere the rows of the y-shells come first (ys rows of nx cells), then the xs = 0, 3 or 6
+  // x-shell cells of each remaining row. n >= 6 keeps the low and high shell of an axis apart.
+  const bool zsh = ((p.shell & 16u) && k < NG) || ((p.shell & 32u) && k >= p.nz - NG);
+  const int ylo = (p.shell & 4u) ? NG : 0, yhi = (p.shell & 8u) ? NG : 0, ys = zsh ? p.ny : ylo + yhi;
+  const int xlo = (p.shell & 1u) ? NG : 0, xs = xlo + ((p.shell & 2u) ? NG : 0);
+  const int nrow = ys * p.nx, ncell = nrow + (p.ny - ys) * xs;
+  for (int q = threadIdx.x; q < ncell; q += blockDim.x) {
+    int i, j;
+    if (q < nrow) {
+      const int r = q / p.nx;
+      i = q - r * p.nx;
+      j = (zsh || r < ylo) ? r : p.ny - NG + (r - ylo);
+    } else {
+      const int r = (q - nrow) / xs, c = (q - nrow) - r * xs;
+      j = ylo + r;
+      i = c < xlo ? c : p.nx - NG + (c - xlo);
+    }
     const long long c = fo + (long long)(k + NG) * p.sz + (long long)(j + NG) * p.pitch + (i + NG);
     const double* uc = u_in + c;
     const double x = G.origin[ip][0] + (double)i * h, y = G.origin[ip][1] + (double)j * h;
@@ -716,6 +731,33 @@ static unsigned shell_bits(const sacra_boundary_t& b) {
     if (b.face[a] == SACRA_BC_SOMMERFELD) s |= 1u << a;
   return s;
 }
+// Eq. 13 divides by r: a cell of a Sommerfeld shell that sits exactly at the coordinate origin (r = 0 in the kernel's
+// own arithmetic, x = origin + i h with a rounded product) would put NaN into u_out and acc without any error.
+// Checked on the host before anything is launched (sacra.h: "the origin of the coordinates must not be a cell of a
+// boundary shell").
+static int check_shell_origin(const sacra_patch_t* p, const sacra_boundary_t* bnd, int npatch) {
+  for (int q = 0; q < npatch; ++q) {
+    const unsigned s = shell_bits(bnd[q]);
+    if (!s) continue;
+    const int n[3] = {p[q].nx, p[q].ny, p[q].nz};
+    int zero[3] = {-1, -1, -1};   // index of the cell whose coordinate along the axis is exactly 0, if any
+    for (int a = 0; a < 3; ++a) {
+      const double g = -bnd[q].origin[a] / p[q].dx;
+      if (!(g > -1.0 && g < (double)n[a])) continue;
+      for (long long i = (long long)g - 1; i <= (long long)g + 2; ++i) {
+        if (i < 0 || i >= n[a]) continue;
+        volatile double prod = (double)i * p[q].dx;   // rounded product, as the kernel forms it (no FMA there)
+        if (bnd[q].origin[a] + prod == 0.0) zero[a] = (int)i;
+      }
+    }
+    if (zero[0] < 0 || zero[1] < 0 || zero[2] < 0) continue;
+    bool hit = false;
+    for (int a = 0; a < 3; ++a)
+      hit = hit || ((s >> (2 * a) & 1u) && zero[a] < NG) || ((s >> (2 * a + 1) & 1u) && zero[a] >= n[a] - NG);
+    if (hit) return SACRA_ERR_BADARG;
+  }
+  return SACRA_OK;
+}
 
 // Sommerfeld shell of every patch that has one: EPI 0 stores the RHS into `rhs`, 1..5 apply the RK4 stage table
 static int launch_sommerfeld(const sacra_patch_t* p, int npatch, const sacra_boundary_t* bnd, int epi, const double* u_in,
@@ -1032,6 +1074,7 @@ int sacra_sommerfeld_rhs(const sacra_patch_t* p, int npatch, const sacra_boundar
   if (!p || !u || !rhs || !bnd) return SACRA_ERR_NULL;
   if (int e = check_patches(p, npatch)) return e;
   if (int e = check_boundaries(bnd, npatch)) return e;
+  if (int e = check_shell_origin(p, bnd, npatch)) return e;
   if (!aligned16(u) || !aligned16(rhs)) return SACRA_ERR_ALIGN;
   const long long ext = state_extent(p, npatch);
   if (overlap(u, ext, rhs, ext)) return SACRA_ERR_BADARG;
@@ -1043,6 +1086,7 @@ int sacra_rk4_substep_bc(const sacra_patch_t* p, int npatch, const sacra_params_
   if (!p || !prm || !bnd || !u_n || !u_in || !u_out || !acc) return SACRA_ERR_NULL;
   if (int e = check_patches(p, npatch)) return e;
   if (int e = check_boundaries(bnd, npatch)) return e;
+  if (int e = check_shell_origin(p, bnd, npatch)) return e;
   if (stage < 1 || stage > 4) return SACRA_ERR_BADARG;
   if (!aligned16(u_n) || !aligned16(u_in) || !aligned16(u_out) || !aligned16(acc)) return SACRA_ERR_ALIGN;
   const long long ext = state_extent(p, npatch);
@@ -1062,6 +1106,7 @@ int sacra_rk4_step_bc(const sacra_patch_t* p, int npatch, const sacra_params_t* 
   if (!p || !prm || !bnd || !u || !work) return SACRA_ERR_NULL;
   if (int e = check_patches(p, npatch)) return e;
   if (int e = check_boundaries(bnd, npatch)) return e;
+  if (int e = check_shell_origin(p, bnd, npatch)) return e;
   if (state_doubles < 1 || (state_doubles & 1) || state_extent(p, npatch) > state_doubles) return SACRA_ERR_BADARG;
   if (!aligned16(u) || !aligned16(work)) return SACRA_ERR_ALIGN;
   if (overlap(u, state_doubles, work, 3 * state_doubles)) return SACRA_ERR_BADARG;
@@ -1267,6 +1312,7 @@ int sacra_subcycle_step(const sacra_patch_t* parent, const sacra_patch_t* child,
   if (!prm || !parent_bnd || !u_parent || !u_parent_prev || !u_child || !work_parent || !work_child) return SACRA_ERR_NULL;
   if (int e = check_levels(parent, child, org, true)) return e;
   if (int e = check_boundaries(parent_bnd, 1)) return e;
+  if (int e = check_shell_origin(parent, parent_bnd, 1)) return e;
   if (std::fabs(2.0 * child->dt - parent->dt) > 1e-12 * std::fabs(parent->dt)) return SACRA_ERR_BADARG;   // halved time step
   if (parent_doubles < state_extent(parent, 1) || child_doubles < state_extent(child, 1) || (parent_doubles & 1) ||
       (child_doubles & 1))
@@ -1384,6 +1430,10 @@ int hier_advance(const HierCtx& c, int l, int m) {
     }
   }
   if (l + 1 < c.nlevels) {
+    // stage 4 wrote active cells only: an intermediate level brings its ghosts to the time just reached before its
+    // child advances, whose prolongation box reads them when the child sits within 4 cells of this level's edge
+    // (level 0: sacra_rk4_step_bc ended with its fill)
+    if (l > 0 && (e = hier_parent_ghosts(c, l, ((double)m + 1.0) / 2.0, me.u))) return e;
     if ((e = hier_advance(c, l + 1, 0))) return e;
     if ((e = hier_advance(c, l + 1, 1))) return e;
     sacra_level_t& ch = c.L[l + 1];
@@ -1431,6 +1481,7 @@ int sacra_hierarchy_step(sacra_level_t* levels, int nlevels, const sacra_params_
       }
     }
   }
+  if (int e = check_shell_origin(levels[0].patch, bnd0, 1)) return e;
   HierCtx c{levels, nlevels, prm, bnd0, static_cast<cudaStream_t>(cuda_stream)};
   return hier_advance(c, 0, 0);
 }

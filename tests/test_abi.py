@@ -183,6 +183,25 @@ def test_boundary_argument_checks():
     assert _code(sacra.rk4_step_bc, ps, PRM, None, FAKE, far, total) == sacra.ERR_NULL
 
 
+def test_sommerfeld_shell_cell_at_the_coordinate_origin_is_rejected():
+    """Eq. 13 divides by r. A cell of a Sommerfeld shell at r = 0 would write NaN without an error, so every call
+    that evaluates Eq. 13 refuses it on the host (8^3 patch, dx = 0.1: the shell of the x- face is i < 3)."""
+    ps, total = _patch()
+    far, som = FAKE + 8 * (total + 64), [2] * 6
+    at = lambda i, j, k: (-0.1 * i, -0.1 * j, -0.1 * k)          # origin that puts cell (i, j, k) at x = y = z = 0
+    for cell in ((0, 0, 0), (2, 4, 4), (4, 4, 7), (3, 5, 4)):
+        assert _code(sacra.sommerfeld_rhs, ps, [(at(*cell), som)], FAKE, far) == sacra.ERR_BADARG, cell
+    # the same cell is fine when it is not in a shell: interior cell, or the face it is near is not a Sommerfeld face
+    for cell, faces in (((4, 4, 4), som), ((3, 3, 4), som), ((0, 4, 4), [1, 2, 2, 2, 2, 2]), ((4, 4, 4), [1] * 6)):
+        assert _code(sacra.sommerfeld_rhs, ps, [(at(*cell), faces)], FAKE, FAKE + 64) == sacra.ERR_BADARG   # reaches the overlap check
+        assert _code(sacra.sommerfeld_rhs, ps, [(at(*cell), faces)], FAKE, far + 8) == sacra.ERR_ALIGN      # ... and the alignment check
+    # an origin that is merely close to a shell cell is accepted (r > 0)
+    assert _code(sacra.sommerfeld_rhs, ps, [((1e-300, 0.0, 0.0), som)], FAKE, far + 8) == sacra.ERR_ALIGN
+    bad = [(at(1, 1, 1), som)]
+    assert _code(sacra.rk4_substep_bc, ps, PRM, bad, 1, FAKE, FAKE, far, far + 8 * (total + 64)) == sacra.ERR_BADARG
+    assert _code(sacra.rk4_step_bc, ps, PRM, bad, FAKE, far, total) == sacra.ERR_BADARG
+
+
 def test_subcycling_argument_checks():
     pp, tp = wl.make_layout([(16, 16, 16)], [0.2], [0.05], [(0, 0, 0)])
     pc, tc = wl.make_layout([(8, 8, 8)], [0.1], [0.025], [(0, 0, 0)])

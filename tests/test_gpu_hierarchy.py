@@ -49,8 +49,11 @@ def test_two_levels_equal_the_pair_step_bitwise():
     assert counts == [2, 4] and np.array_equal(host(pv[0]), host(prev))
 
 
-def test_three_levels_against_the_oracle_recursion():
-    ws, orgs, bnd = hierarchy(16, 3, _data(seed=6))
+@pytest.mark.parametrize("org2", [None, 2, 6])
+def test_three_levels_against_the_oracle_recursion(org2):
+    """org2 = 2, 6: an off-centre grandchild, whose prolongation box reaches into level 1's ghost cells (they must be at
+    the new time before level 2 advances; pinned on the oracle in test_oracle_hierarchy.py)"""
+    ws, orgs, bnd = hierarchy(16, 3, _data(seed=6), org=None if org2 is None else [0, 4, org2])
     ps = [w.patches[0] for w in ws]
     prm = ws[0].params
     st, pv, wk = _gpu_levels(ws)
@@ -58,6 +61,7 @@ def test_three_levels_against_the_oracle_recursion():
     ref = [w.state.copy() for w in ws]
     rprev = [np.zeros_like(s) for s in ref]
     rcount = [0, 0, 0]
+    worst = 0.0
     for step in range(2):
         before = [r.copy() for r in ref]
         orc.hierarchy_step(ps, orgs, prm, bnd, ref, rprev, rcount)
@@ -72,4 +76,32 @@ def test_three_levels_against_the_oracle_recursion():
                 rate = np.max(np.abs(b - w.field_view(before[l], 0, f)[:, :, :q.nx + 2 * NG])) / (q.dt * 2 ** l)
                 tol = 16 * (step + 1) * (q.dt * 2 ** l) * RTOL * (rate + FLOOR) + 4 * np.spacing(np.max(np.abs(b)))
                 assert np.max(np.abs(a - b)) <= tol, (step, l, wl.FIELD_NAMES[f], np.max(np.abs(a - b)), tol)
+                worst = max(worst, np.max(np.abs(a - b)) / tol)
+    print("\n[tolerance use] three levels (org2 = %s), 2 coarse steps: worst max|d| / tol = %.3f" % (org2, worst))
     assert np.max(np.abs(ws[2].active_view(ref[2], 0, wl.F_G + 3) - ws[2].active_view(ws[2].state, 0, wl.F_G + 3))) > 1e-6
+
+
+@pytest.mark.parametrize("org2", [2, 3])
+def test_off_centre_grandchild_linear_in_time_on_the_gpu(org2):
+    """the oracle's pin of the same name, on the CUDA path: beta^i = b0 + 0.75 B0 t to round-off on all three levels,
+    ghosts included (3e-3 at org 2 if level 1's ghosts are still at the old time when level 2 advances)"""
+    B0, b0 = np.array([0.3, -0.2, 0.1]), np.array([0.05, 0.02, -0.04])
+    def fn(X, Y, Z):
+        v = _flat(X)
+        for i in range(3):
+            v[wl.F_B + i] = np.full_like(X, B0[i]); v[wl.F_BET + i] = np.full_like(X, b0[i])
+        return v
+    ws, orgs, bnd = hierarchy(16, 3, fn, h=0.5, org=[0, 4, org2])
+    prm = dict(ws[0].params, eta=0.0)
+    ps = [w.patches[0] for w in ws]
+    st, pv, wk = _gpu_levels(ws)
+    counts = [0, 0, 0]
+    for step in (1, 2):
+        sacra.hierarchy_step(ps, orgs, prm, bnd, st, pv, wk, counts)
+        t = step * ps[0].dt
+        for l, w in enumerate(ws):
+            got = host(st[l])
+            for i in range(3):
+                a = w.field_view(got, 0, wl.F_BET + i)[:, :, :ps[l].nx + 2 * NG]
+                want = b0[i] + 0.75 * B0[i] * t
+                assert np.max(np.abs(a - want)) < 6e-16, (step, l, i, np.max(np.abs(a - want)))
