@@ -128,14 +128,14 @@ def rk4_step_distributed(patch, params, u, work, topo: CartTopology, rank: int, 
         buffers["comm_stream"] = torch.cuda.Stream()
     comm = buffers["comm_stream"]
     faces = [1] * 6                      # every face of a block of a periodic decomposition is an exchange face
-    cops = ops or CudaOps()
+    # the overlapped exchanges pack / unpack on the second stream through an ops object of their own: the caller's
+    # `ops` (and whatever stream it carries) is left as it was and serves the final exchange below
+    comm_ops = CudaOps(comm) if ops is None or isinstance(ops, CudaOps) else ops
     for stage, (src, dst) in enumerate(seq, start=1):
         comm.wait_stream(main)           # the stage input is complete
         with torch.cuda.stream(comm):
-            cops.stream = comm
-            exchange_halos(patch, src, topo, rank, cops, group, buffers)
+            exchange_halos(patch, src, topo, rank, comm_ops, group, buffers)
         sacra.rk4_substep_part([patch], params, stage, sacra.PART_INTERIOR, faces, u, src, dst, acc)
         main.wait_stream(comm)           # ghosts of the stage input are in place
         sacra.rk4_substep_part([patch], params, stage, sacra.PART_SHELL, faces, u, src, dst, acc)
-    cops.stream = None
-    exchange_halos(patch, u, topo, rank, cops, group, buffers)
+    exchange_halos(patch, u, topo, rank, ops, group, buffers)
