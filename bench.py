@@ -36,6 +36,18 @@ ALG_BYTES_PER_POINT_STEP = 16 * 8 * NF
 ALG_FLOP_PER_POINT_STAGE = 4195.0
 ALG_FP64_INSTR_PER_POINT_STAGE = 3206.0
 FP64_LANES_PER_SM, N_SM = 64, 148
+# The count SURVEY 8(d) asks for, beside the SASS one: the oracle's point-wise algebra instantiated with an
+# operation-counting scalar (1 787 add + 1 777 mul + 12 div = 3 576, no CSE; tests/test_bench_counts.py checks the number
+# against orc.count_ops()) plus the needed derivative operators in canonical form with shared inner differences
+# (48 D1 x 5 + 33 D_aa x 9 + 33 D_ab x 5 + 25 upwind x 41 + 25 KO x 42 = 2 777). The roofline
+# fraction is credited with the SMALLER of the two counts (the SASS one).
+ORACLE_ALGEBRA_OPS = 1787 + 1777 + 12
+CANONICAL_DERIVATIVE_OPS = 48 * 5 + 33 * 9 + 33 * 5 + 25 * 41 + 25 * 42
+ORACLE_FLOP_PER_POINT_STAGE = float(ORACLE_ALGEBRA_OPS + CANONICAL_DERIVATIVE_OPS)
+# Measured FP64 rate of this pool's B200 (BASELINE.md section 3, round-1 register-chain microbenchmark at 1 965 MHz):
+# DFMA 17.06 Tinst/s = 34.1 TFLOP/s (58.7 of the 64 lanes per SM and clock); scaled with the SM clock of the run.
+FP64_MEASURED_TFLOPS, FP64_MEASURED_AT_MHZ = 34.1, 1965.0
+TIMED_FLAGS = ["SKIP_INCREMENT"]     # sacra_params_t.flags of every timed step (not the library default, see run_ours)
 
 
 def _peaks():
@@ -156,22 +168,37 @@ def time_oracle(sample, steps, warmup):
     return ts, orc.num_threads()
 
 
+def config_of(w, world: int):
+    """the `config` object of the JSON line: the same for both arms, so that they can be compared key by key"""
+    state_bytes = w.state.size * 8
+    return {"workload": w.name, "patches": len(w.patches), "points": w.npoints, "fields": NF, "ghosts": 3,
+            "state_bytes": state_bytes, "l2": "state (%.2f GB) larger than L2; no flush needed" %
+            (state_bytes / 1e9) if state_bytes > 2.6e8 else "state fits L2: numbers are L2-resident",
+            "parallelism": "replicas only" if world > 1 else "1 GPU"}
+
+
 def run_reference(args):
+    """the oracle, as it stands, on the host cores. Without --oracle-n it advances the WHOLE workload (config 4: the full
+    256^3 patch, about 10 s per RK4 step on 16 cores), so both arms run the same configuration; --oracle-n M bounds it
+    to the central M^3 block (the sample of the cpu_baseline leg)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     w = make_workload(args.config, args.n)
-    m = args.oracle_n or ORACLE_SAMPLE_N
-    s = oracle_sample(w, m)
+    if args.oracle_n:
+        s = oracle_sample(w, args.oracle_n)
+        what = "central %d^3 block of %s as a periodic patch" % (s.patches[0].nx, w.name)
+    else:
+        s, what = w, "the whole of %s" % w.name
     ts, cores = time_oracle(s, args.steps, args.warmup)
     tot = sum(ts)
     val = s.npoints * len(ts) / tot / 1e6
-    sample = "central %d^3 block of %s as a periodic patch, %d RK4 steps" % (s.patches[0].nx, w.name, len(ts))
+    sample = "%s, %d RK4 steps" % (what, len(ts))
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(ts),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "sample": sample},
+        "config": config_of(w, int(os.environ.get("WORLD_SIZE", "1"))),
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -240,6 +267,17 @@ def run_ours(args):
     clocks = sampler.stop(t0, t1) if rank == 0 else None
     if not bool(torch.isfinite(u).all()):
         raise SystemExit("bench.py: non-finite state after the timed steps")
+    # the same K steps with the library's default flags (stage 4 also stores S): reported beside the headline
+    prm_default = sacra.make_params(dict(w.params, flags=0))
+    sacra.rk4_step(ps, prm_default, u, work, n)
+    d0, d1 = ev(), ev()
+    barrier()
+    d0.record(stream)
+    for s in range(K):
+        sacra.rk4_step(ps, prm_default, u, work, n)
+    d1.record(stream)
+    barrier()
+    default_flags_ms = max_over_ranks(d0.elapsed_time(d1)) / K
 
     # ---- kernel split for the roofline: same nine calls, CUDA events around each -----------------------
     a, b, acc = work[:n], work[n:2 * n], work[2 * n:]
@@ -344,16 +382,27 @@ def run_ours(args):
     # roofline of the dominant kernel (the fused substage kernel), per launch, averaged over the 4 stages
     alg_bytes = ALG_BYTES_PER_POINT_STEP / 4.0 * npts
     alg_flop = ALG_FLOP_PER_POINT_STAGE * npts
-    fp64_peak_tf = N_SM * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    fp64_peak_tf = N_SM * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12          # nominal
+    fp64_meas_tf = FP64_MEASURED_TFLOPS * sm_max_mhz / FP64_MEASURED_AT_MHZ         # measured DFMA rate
     t_hbm = alg_bytes / (hbm_gbs * 1e9)
-    t_alu = alg_flop / (fp64_peak_tf * 1e12)
+    t_alu = alg_flop / (fp64_meas_tf * 1e12)
     t_k = sub_avg * 1e-3
+    # the metric's roofline: the slower of the compulsory bytes at the measured HBM rate and the flops at the MEASURED
+    # FP64 rate; the nominal FP64 peak and both fractions are reported beside it
     if t_alu >= t_hbm:
-        roof = {"bound": "alu", "achieved": alg_flop / t_k / 1e12, "peak": fp64_peak_tf, "unit": "TFLOP/s"}
+        roof = {"bound": "alu", "achieved": alg_flop / t_k / 1e12, "peak": fp64_meas_tf, "unit": "TFLOP/s"}
     else:
         roof = {"bound": "hbm", "achieved": alg_bytes / t_k / 1e9, "peak": hbm_gbs, "unit": "GB/s"}
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof.update({
+        "t_hbm_ms": 1e3 * t_hbm, "t_alu_ms": 1e3 * t_alu, "t_alu_nominal_ms": 1e3 * alg_flop / (fp64_peak_tf * 1e12),
+        "alu_peak_measured_tflops": fp64_meas_tf, "alu_peak_nominal_tflops": fp64_peak_tf,
+        "alu_frac_measured_peak": (alg_flop / t_k / 1e12) / fp64_meas_tf,
+        "alg_flop_per_point_stage": {"credited": ALG_FLOP_PER_POINT_STAGE,
+                                     "kernel_sass_fma2": ALG_FLOP_PER_POINT_STAGE,
+                                     "oracle_counting_scalar": ORACLE_FLOP_PER_POINT_STAGE,
+                                     "note": "oracle: algebra %d ops (no CSE) + needed derivative operators %d; the "
+                                             "smaller count is credited" % (ORACLE_ALGEBRA_OPS, CANONICAL_DERIVATIVE_OPS)},
         "traffic": args.traffic if args.traffic is not None else _committed_traffic(w.name),
         "traffic_source": "profiles/r02_traffic.json (ncu dram__bytes_read.sum + dram__bytes_write.sum, mean of the four "
                           "substage launches; null if the kernel sources changed since the capture)",
@@ -365,7 +414,8 @@ def run_ours(args):
         # ceiling of this instruction mix (a quarter FMAs); measured DFMA/DADD rates: BASELINE.md section 3
         "fp64_issue_frac": ALG_FP64_INSTR_PER_POINT_STAGE * npts / t_k /
                            (N_SM * FP64_LANES_PER_SM * sm_max_mhz * 1e6),
-        "peak_source": peak_src + "; FP64 peak = 148 SM x 64 lanes x 2 x sm_max_mhz (DESIGN.md)"})
+        "peak_source": peak_src + "; FP64: measured DFMA rate 34.1 TFLOP/s at 1 965 MHz (BASELINE.md section 3) scaled "
+                       "to sm_max_mhz; nominal = 148 SM x 64 lanes x 2 x sm_max_mhz (DESIGN.md section 7)"})
 
     # ---- CPU oracle beside it (reported baseline, bounded sample) -----------------------------------------
     cpu = None
@@ -379,15 +429,16 @@ def run_ours(args):
                          % (s.patches[0].nx, w.name, len(ts), sum(ts))}
 
     state_bytes = n * 8
+    cfg = config_of(w, world)
     ghost_cells = sum((p.nx + 6) * (p.ny + 6) * (p.nz + 6) - p.nx * p.ny * p.nz for p in w.patches)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": total_ms / K, "ms_per_step_min": min(step_ms), "ms_per_step_median": sorted(step_ms)[K // 2],
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "patches": len(w.patches), "points": npts, "fields": NF, "ghosts": 3,
-                   "state_bytes": state_bytes, "l2": "state (%.2f GB) larger than L2; no flush needed" %
-                   (state_bytes / 1e9) if state_bytes > 2.6e8 else "state fits L2: numbers are L2-resident",
-                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "config": cfg,
+        # sacra_params_t.flags of every timed step (value, e2e, roofline split, configs 0-3): stage 4 does not store the
+        # increment S, one field pass less per step than the library default; the new state is the same bit for bit
+        "flags": TIMED_FLAGS, "ms_per_step_default_flags": default_flags_ms,
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes,
                 "ms_per_step": e2e_ms / K, "how": "pinned host state in and out every step; independent jobs, two device "
                 "buffers, copy-in / kernels / copy-out on three streams",
@@ -402,7 +453,7 @@ def run_ours(args):
                                "norms_H_Mx_My_Mz": norms_host},
     }
     if args.all_configs and world == 1 and args.config == 4 and not args.n:
-        out["configs"] = [measure_config(i, args, hbm_gbs, fp64_peak_tf) for i in range(4)]
+        out["configs"] = [measure_config(i, args, hbm_gbs, fp64_meas_tf) for i in range(4)]
     print(json.dumps(out))
 
 
