@@ -90,6 +90,7 @@ def test_ten_consecutive_steps_beside_the_oracle(idx, nsteps, quad_steps):
             tol = 1e-9 * abs(no[c]) + 4.0 * abs(nb[c] - no[c]) + 1e-15
             assert abs(ng[c] - no[c]) <= tol, (w.name, "norm", k, c, ng[c], no[c], tol)
     assert worst > 0.0 or idx == 0
+    print("\n[tolerance use] %s, %d steps: worst max|d| / bound = %.3f" % (w.name, nsteps, worst))
 
 
 def test_skip_increment_flag_gives_the_same_state_bitwise():
@@ -131,6 +132,13 @@ def test_full_size_config4_all_points_against_oracle():
     chk = got.copy()
     orc.fill_ghosts(w.patches, chk)
     assert np.array_equal(chk, got)          # ghosts of the result are filled
+    # the step bench.py TIMES sets SACRA_FLAG_SKIP_INCREMENT (stage 4 is k_z4c<5>, not <4>): same size, same launch
+    # shape, and the new state must be the one just checked, bit for bit, ghosts and padding included
+    u = dev(w.state)
+    n = u.numel()
+    work = torch.zeros(3 * n, dtype=torch.float64, device="cuda")
+    sacra.rk4_step(w.patches, dict(w.params, flags=sacra.FLAG_SKIP_INCREMENT), u, work)
+    assert np.array_equal(host(u), got)
 
 
 def test_repeatable_bit_for_bit_with_guard_bands():

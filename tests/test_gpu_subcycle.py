@@ -62,6 +62,7 @@ def test_two_subcycle_steps_against_the_oracle_driver():
     gp, gc, gprev = dev(P.state), dev(Cw.state), torch.zeros(P.state.size, dtype=torch.float64, device="cuda")
     wp = torch.zeros(5 * P.state.size, dtype=torch.float64, device="cuda")
     wc = torch.zeros(3 * Cw.state.size, dtype=torch.float64, device="cuda")
+    worst = 0.0
     for step in range(2):
         before = (up.copy(), uc.copy())
         g_before = host(gp).copy()
@@ -75,6 +76,8 @@ def test_two_subcycle_steps_against_the_oracle_driver():
                 rate = np.max(np.abs(b - w.field_view(old, 0, f)[:, :, :q.nx + 2 * NG])) / q.dt   # ~ max|S_f|
                 tol = 8 * (step + 1) * q.dt * RTOL * (rate + FLOOR) + 4 * np.spacing(np.max(np.abs(b)))
                 assert np.max(np.abs(a - b)) <= tol, (step, w.name, wl.FIELD_NAMES[f], np.max(np.abs(a - b)), tol)
+                worst = max(worst, np.max(np.abs(a - b)) / tol)
         assert np.array_equal(host(gprev), g_before)       # U^n handed back, bit for bit (a copy)
+    print("\n[tolerance use] pair, 2 coarse steps: worst max|d| / tol = %.3f" % worst)
     # the child did move, and the parent's covered cells are the restriction of the child (not the parent's own step)
     assert np.max(np.abs(Cw.active_view(uc, 0, wl.F_G + 3) - Cw.active_view(Cw.state, 0, wl.F_G + 3))) > 1e-6
