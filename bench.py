@@ -7,7 +7,9 @@ One "step" = one full RK4 step (5 halo fills + 4 fused RHS/KO/RK substages) of t
 C ABI call sacra_rk4_step. Default workload: BASELINE.json configs[4], one 256^3 periodic patch, 25 FP64 fields,
 Brill-Lindquist data + 1e-12 seeded noise (the configuration the north_star target is stated on; it fits one
 GPU). N > 1 (torchrun): "replicas only" -- every rank advances its own independent 256^3 patch, no data-path
-collective (Multi-GPU); value = points of all ranks / max-over-ranks time.
+collective (Multi-GPU); value = points of all ranks / max-over-ranks time. With --decomp PXxPYxPZ the N
+ranks instead share ONE periodic domain, a 256^3 block each, and exchange 3-layer halos over NCCL before every substage
+(run_decomp).
 
 Prints ONE JSON line (rank 0). Keys: see DESIGN.md "Measurement".
 """
@@ -71,9 +73,9 @@ def _csrc_digest() -> str:
 
 
 def _committed_traffic(workload: str):
-    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/r02_traffic.json), or None
+    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/r03_traffic.json), or None
     when the capture was made for other kernel sources or another workload"""
-    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    p = os.path.join(ROOT, "profiles", "r03_traffic.json")
     try:
         d = json.load(open(p))
     except (OSError, ValueError):
@@ -404,7 +406,7 @@ def run_ours(args):
                                      "note": "oracle: algebra %d ops (no CSE) + needed derivative operators %d; the "
                                              "smaller count is credited" % (ORACLE_ALGEBRA_OPS, CANONICAL_DERIVATIVE_OPS)},
         "traffic": args.traffic if args.traffic is not None else _committed_traffic(w.name),
-        "traffic_source": "profiles/r02_traffic.json (ncu dram__bytes_read.sum + dram__bytes_write.sum, mean of the four "
+        "traffic_source": "profiles/r03_traffic.json (ncu dram__bytes_read.sum + dram__bytes_write.sum, mean of the four "
                           "substage launches; null if the kernel sources changed since the capture)",
         "kernel": "k_z4c (fused derivative+algebra+KO+RK substage)",
         "kernel_ms": sub_avg, "kernel_share_of_step": 4 * sub_avg / (4 * sub_avg + 5 * fill_avg),
@@ -455,6 +457,132 @@ def run_ours(args):
     if args.all_configs and world == 1 and args.config == 4 and not args.n:
         out["configs"] = [measure_config(i, args, hbm_gbs, fp64_meas_tf) for i in range(4)]
     print(json.dumps(out))
+
+
+def run_decomp(args):
+    """--decomp PXxPYxPZ: the sharded path of SURVEY 8(f) f-4. PX*PY*PZ = the number of
+    ranks; every rank owns one block of a periodic (n PX) x (n PY) x (n PZ) domain and advances it with
+    halo.rk4_step_distributed: pack -> NCCL point-to-point -> unpack of the 3-layer halos before every substage, overlapped
+    with the interior cells. The domain is the periodic tiling of the workload's patch (config 4: 256^3 per rank), so
+    every rank's block must come out equal, bit for bit, to the single-GPU periodic step of that patch: checked on one
+    step before the timed region (`decomp_check`). Weak scaling: the work per GPU is fixed."""
+    import torch
+    import torch.distributed as dist
+    from paper_2607_08743_b200 import halo, replicas, sacra
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dims = tuple(int(v) for v in args.decomp.lower().split("x"))
+    if len(dims) != 3 or dims[0] * dims[1] * dims[2] != world:
+        raise SystemExit("bench.py: --decomp %s does not match %d ranks" % (args.decomp, world))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libsacra has no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = make_workload(args.config, args.n)
+    if len(w.patches) != 1:
+        raise SystemExit("bench.py: --decomp needs a single-patch workload")
+    p = w.patches[0]
+    prm = dict(w.params, flags=sacra.FLAG_SKIP_INCREMENT)
+    topo = halo.CartTopology(dims)
+    n = w.state.size
+    host_in = torch.from_numpy(w.state).pin_memory()
+    host_out = torch.empty_like(host_in).pin_memory()
+    u = torch.empty(n, dtype=torch.float64, device="cuda")
+    work = torch.zeros(3 * n, dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+    K, W = args.steps, args.warmup
+    bufs = {}
+
+    # one step against the single-GPU periodic step of the same patch: same bits
+    v, wv = torch.from_numpy(w.state).cuda(), torch.zeros(3 * n, dtype=torch.float64, device="cuda")
+    sacra.rk4_step([p], prm, v, wv, n)
+    u.copy_(host_in)
+    halo.rk4_step_distributed(p, prm, u, work, topo, rank, buffers=bufs, overlap=True)
+    torch.cuda.synchronize()
+    same = float(bool(torch.equal(u, v)))
+    same = replicas.sum_over_ranks(same, device="cuda") == world
+    del v, wv
+
+    def ev():
+        return torch.cuda.Event(enable_timing=True)
+
+    def timed(overlap, sampler=None):
+        u.copy_(host_in)
+        for _ in range(W):
+            halo.rk4_step_distributed(p, prm, u, work, topo, rank, buffers=bufs, overlap=overlap)
+        if sampler is not None and rank == 0:
+            sampler.start()
+            time.sleep(0.25)
+        barrier()
+        t0 = time.time()
+        e0, e1 = ev(), ev()
+        e0.record(stream)
+        for _ in range(K):
+            halo.rk4_step_distributed(p, prm, u, work, topo, rank, buffers=bufs, overlap=overlap)
+        e1.record(stream)
+        barrier()
+        ms = replicas.max_over_ranks(e0.elapsed_time(e1), device="cuda")
+        clocks = sampler.stop(t0, time.time()) if sampler is not None and rank == 0 else None
+        return ms, clocks
+
+    # the headline is the mode --overlap names (default off: on one GPU, where every exchange is a local copy, the split
+    # into interior and shell launches costs more than it hides -- 36.0 against 27.1 ms per 256^3 step; DESIGN.md section 9);
+    # the other mode is timed beside it
+    head = args.overlap == "on"
+    other_ms, _ = timed(not head)
+    total_ms, clocks = timed(head, ClockSampler(local))
+    on_ms, plain_ms = (total_ms, other_ms) if head else (other_ms, total_ms)
+    if not bool(torch.isfinite(u).all()):
+        raise SystemExit("bench.py: non-finite state after the timed steps")
+    # end to end: pinned host state in, one distributed step, new state out, every step
+    barrier()
+    e0, e1 = ev(), ev()
+    for it in range(2 + K):
+        if it == 2:
+            barrier()
+            e0.record(stream)
+        u.copy_(host_in, non_blocking=True)
+        halo.rk4_step_distributed(p, prm, u, work, topo, rank, buffers=bufs, overlap=head)
+        host_out.copy_(u, non_blocking=True)
+    e1.record(stream)
+    barrier()
+    e2e_ms = replicas.max_over_ranks(e0.elapsed_time(e1), device="cuda")
+    if world > 1:
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+    npts = w.npoints
+    msgs = 2 * sum(1 for d in dims if d > 1)
+    xbytes = 5 * 2 * 8 * sum(sacra.face_doubles(p, a) for a in range(3) if dims[a] > 1)      # sent per rank and step
+    cfg = config_of(w, world)
+    cfg.update({"parallelism": "3-D blocks %s, 3-layer halo, NCCL p2p, exchange %s" %
+                               (args.decomp, "overlapped with the interior" if head else "before each substage"),
+                "global_domain": [p.nx * dims[0], p.ny * dims[1], p.nz * dims[2]], "points_per_gpu": npts})
+    print(json.dumps({
+        "metric": METRIC, "value": world * npts * K / (total_ms * 1e-3) / 1e6, "unit": UNIT, "n_gpus": world, "steps": K,
+        "warmup": W, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": cfg, "flags": TIMED_FLAGS,
+        "e2e": {"value": world * npts * K / (e2e_ms * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": n * 8,
+                "d2h_bytes_per_step": n * 8, "ms_per_step": e2e_ms / K,
+                "how": "per rank: pinned host state in, one distributed step, new state out, on one stream"},
+        # 4 substage launches (overlap on: interior + shell each) + pack / unpack of 6 faces x 5 exchanges
+        "gpu_launches": K * ((8 if head else 4) + 5 * 12), "clocks": clocks,
+        "halo": {"messages_per_exchange": msgs, "exchanges_per_step": 5, "sent_bytes_per_rank_and_step": xbytes,
+                 "overlap": args.overlap, "ms_per_step_overlap_on": on_ms / K, "ms_per_step_overlap_off": plain_ms / K},
+        "decomp_check": "every rank's block after one step is bit-equal to sacra_rk4_step of the periodic patch: %s"
+                        % ("yes" if same else "NO"),
+        "roofline": None, "cpu_baseline": None}))
+    if not same:
+        raise SystemExit("bench.py: the distributed step differs from the single-GPU periodic step")
 
 
 def measure_config(idx, args, hbm_gbs, fp64_peak_tf):
@@ -516,14 +644,21 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel (default: the committed ncu capture "
-                         "profiles/r02_traffic.json if it was made for the current kernel sources)")
+                         "profiles/r03_traffic.json if it was made for the current kernel sources)")
     ap.add_argument("--all-configs", action="store_true", default=True,
                     help="also time BASELINE.json configs 0-3 (default; the headline stays config 4, the line gains `configs`)")
     ap.add_argument("--headline-only", dest="all_configs", action="store_false", help="skip configs 0-3")
+    ap.add_argument("--decomp", default=None, metavar="PXxPYxPZ",
+                    help="run the sharded path: one block per rank of a periodic domain, halo exchange over NCCL "
+                         "(default: replicas, no exchange)")
+    ap.add_argument("--overlap", default="off", choices=["on", "off"],
+                    help="--decomp: which mode the headline times (the other one is reported under `halo`)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.decomp:
+        run_decomp(args)
     else:
         run_ours(args)
 
